@@ -1,0 +1,130 @@
+/*
+ * ovl.h -- C-ABI boundary of the B200-native overlap Dirac operator hot path of arXiv 1510.06897
+ *          (Cundy & Lee, "Overlap fermions on GPUs").  PAPER.md = /root/reference/PAPER.md.
+ *
+ * What the library computes (every step runs in hand-written sm_100a kernels; there is no CPU fallback):
+ *     y = D[mu] psi = 1/2 (1 + mu + (1 - mu) gamma5 sign(K)) psi                    eq. 2.1
+ *     K = gamma5 (D_W - m_w),  m_w = 1.5
+ *     (D_W psi)(x) = 4 psi(x) - 1/2 sum_mu [ (1 - gamma_mu) U_mu(x) psi(x + mu)
+ *                                          + (1 + gamma_mu) U_mu(x - mu)^dag psi(x - mu) ]
+ *                                                                 eq. 2.2, PAPER.md:41 (reading R1)
+ *     sign(K) psi ~= sum_{m=0}^{N} alpha_m T_m(K^) psi
+ *                    + sum_i phi_i (phi_i^dag psi) [ sign(lambda_i) - sum_m alpha_m T_m(lambda_i / lambda_max) ]
+ *                    with K^ = K / lambda_max                     eq. 2.3, PAPER.md:62-64 (reading R5)
+ *     CG on D[mu]^dag D[mu] x = b                                 BASELINE.json north_star (d) (R13, R14)
+ *
+ * Conventions:
+ *   dims = {Lx, Ly, Lz, Lt}, every extent >= 2; V = Lx Ly Lz Lt; site index s = x + Lx (y + Ly (z + Lz t)).
+ *   Canonical spinor:  [V][spin 4][colour 3] complex, interleaved (re, im).  complex128 when the context was
+ *                      created with OVL_F64, complex64 with OVL_F32.
+ *   Canonical links:   [V][mu = x,y,z,t][row 3][col 3] complex128, U_mu(x) being exactly the matrix that multiplies
+ *                      psi(x + mu) in eq. 2.2.  NO boundary phase folded in: the library applies periodic x,y,z and
+ *                      antiperiodic t (the hop across the t boundary carries -1, reading R3).
+ *   Eigenvectors:      [nev][V][4][3] complex128 (always fp64 at the boundary; rounded to fp32 inside for OVL_F32).
+ *   gamma basis:       Euclidean Hermitian chiral (DeGrand-Rossi), gamma5 = diag(+1,+1,-1,-1) (reading R2,
+ *                      tests/golden/gamma_basis.txt).
+ *
+ * Pointers.  Every `const void *` / `void *` data argument marked [H|D] may be a device pointer (used in place) or
+ *   a host pointer (pageable or pinned; the library stages it through its own device buffer with cudaMemcpyAsync on
+ *   the context stream and, for outputs, synchronises before returning).  The kind is detected with
+ *   cudaPointerGetAttributes.  `alpha`, `lambda`, `dims` and the scalar out-parameters are host memory.
+ *
+ * Ownership.  The caller owns everything it passes in; the library never frees or keeps caller pointers.  Links and
+ *   eigenvectors are re-laid-out into context-owned device memory (cudaMalloc) at create / set time, so the
+ *   caller may release them afterwards.  `out` must not alias `psi`.
+ *
+ * Execution.  All work is enqueued on the stream given to ovl_create.  Calls with device outputs return without
+ *   synchronising; ovl_cg, ovl_destroy and any call with a host output synchronise the stream.  A context is
+ *   not thread-safe.  Same inputs => bit-identical outputs run to run (fixed reduction trees, no float atomics).
+ *
+ * Errors.  Every function returns an OVL_* status; nothing throws or prints.  ovl_last_error gives a
+ *   human-readable message for the last non-OK status of that context.
+ */
+#ifndef OVL_H
+#define OVL_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ovl_ctx ovl_ctx; /* opaque */
+
+enum { OVL_OK = 0, OVL_EINVAL = 1, OVL_ENOMEM = 2, OVL_ECUDA = 3, OVL_ESTATE = 4, OVL_ENOTCONV = 5 };
+enum { OVL_F64 = 0, OVL_F32 = 1 };        /* storage + stencil arithmetic precision (reading R18) */
+enum { OVL_RECON18 = 18, OVL_RECON12 = 12 }; /* reals stored per link; 12: third row rebuilt as conj(r0 x r1) */
+
+/* Library version string, e.g. "ovl-b200 0.1 (sm_100a)". */
+const char *ovl_version(void);
+
+/* Device bytes a context for this configuration allocates (links + work vectors + max_nev eigenvectors). */
+size_t ovl_device_bytes(const int dims[4], int prec, int recon, int max_nev);
+
+/* Create a context: re-lay-out the links (S2; SoA site-coalesced planes, optional 12-real compression) and
+ * allocate the recurrence workspace (S4: "short three vector recurrence").
+ *   links_c128 [H|D]  canonical links, V*4*9 complex128.
+ *   cuda_stream       a cudaStream_t (0 = legacy default stream); all later work is enqueued there.
+ * Defaults: m_w = 1.5, lambda_max = 8 - m_w = 6.5 (reading R5); no polynomial, no deflation.
+ * Errors: OVL_EINVAL (null pointer, extent < 2, unknown prec/recon), OVL_ENOMEM, OVL_ECUDA. */
+int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int prec, int recon, void *cuda_stream);
+
+/* Synchronise the stream and free everything the context owns. */
+int ovl_destroy(ovl_ctx *ctx);
+
+/* K = gamma5 (D_W - m_w), K^ = K / lambda_max (R5).  lambda_max > 0. */
+int ovl_set_kernel(ovl_ctx *ctx, double m_w, double lambda_max);
+
+/* Chebyshev table of eq. 2.3: alpha[0..degree_N] (host, fp64), degree_N >= 1.  The recurrence is run up to the
+ * last non-zero alpha (reading R7); ovl_poly_orders reports that number of K^ applications. */
+int ovl_set_chebyshev(ovl_ctx *ctx, int degree_N, const double *alpha);
+int ovl_poly_orders(const ovl_ctx *ctx);
+
+/* Deflation space of eq. 2.3: nev >= 0 vectors phi_c128 [H|D] and eigenvalues lambda (host).
+ * nev = 0 switches deflation off.  |lambda_i| < 1e-14 lambda_max is rejected with OVL_EINVAL (reading R9).
+ * The vectors are used exactly as given (no re-orthonormalisation; reading R10). */
+int ovl_set_deflation(ovl_ctx *ctx, int nev, const void *phi_c128, const double *lambda);
+
+/* out = D_W psi, eq. 2.2 (no m_w shift, no gamma5).  psi, out [H|D] canonical spinors. */
+int ovl_dw(ovl_ctx *ctx, const void *psi, void *out);
+
+/* out = K^ psi = gamma5 (D_W - m_w) psi / lambda_max (one fused stencil pass). */
+int ovl_khat(ovl_ctx *ctx, const void *psi, void *out);
+
+/* out = sign(K) psi by eq. 2.3 (needs ovl_set_chebyshev; OVL_ESTATE otherwise). */
+int ovl_sign(ovl_ctx *ctx, const void *psi, void *out);
+
+/* out = D[mu] psi (dagger = 0, eq. 2.1) or D[mu]^dag psi = 1/2 [(1+mu) psi + (1-mu) sign(K) gamma5 psi]
+ * (dagger = 1, reading R12). */
+int ovl_overlap(ovl_ctx *ctx, double mu, int dagger, const void *psi, void *out);
+
+/* Conjugate gradient on D[mu]^dag D[mu] x = b, x0 = 0, stop when the recursive residual ||r_k|| <= tol ||b||
+ * or after maxiter iterations (tol <= 0: exactly maxiter iterations, status OVL_OK).  b, x [H|D] canonical.
+ * *iters_out = iterations done, *true_relres_out = ||b - A x|| / ||b|| recomputed at the end.
+ * Returns OVL_ENOTCONV (x = last iterate) if tol > 0 was not reached.  Synchronises. */
+int ovl_cg(ovl_ctx *ctx, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out,
+           double *true_relres_out);
+
+const char *ovl_last_error(const ovl_ctx *ctx);
+
+/* ---- native-layout fields (benchmark / solver plumbing: no relayout passes inside the timed calls) -------------
+ * A native field is an opaque device buffer of ovl_field_bytes(ctx) bytes owned by the caller (device memory). */
+size_t ovl_field_bytes(const ovl_ctx *ctx);
+int ovl_field_import(ovl_ctx *ctx, const void *canonical /*[H|D]*/, void *native /*D*/);
+int ovl_field_export(ovl_ctx *ctx, const void *native /*D*/, void *canonical /*[H|D]*/);
+int ovl_dw_native(ovl_ctx *ctx, const void *in_native, void *out_native);
+int ovl_overlap_native(ovl_ctx *ctx, double mu, int dagger, const void *in_native, void *out_native);
+
+/* ---- measurement hooks ------------------------------------------------------------------------------------------
+ * With profiling on, ovl_sign / ovl_overlap(_native) bracket the polynomial loop (the launches of the fused
+ * Wilson+Chebyshev kernel) with CUDA events on the context stream.  ovl_last_poly_timing synchronises
+ * those events and returns the loop's device time in ms and the number of fused-kernel launches in it. */
+int ovl_set_profiling(ovl_ctx *ctx, int on);
+int ovl_last_poly_timing(ovl_ctx *ctx, float *ms_out, int *launches_out);
+/* Total kernels this context has launched since creation (bench.py's gpu_launches). */
+long long ovl_launch_count(const ovl_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OVL_H */

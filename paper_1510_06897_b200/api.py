@@ -1,0 +1,120 @@
+"""Convenience wrapper over the C-ABI binding: owns an ovl_ctx, allocates outputs, accepts torch tensors
+(CUDA or CPU) and numpy arrays.  Argument plumbing only -- every operation is one call into libovl.so."""
+from __future__ import annotations
+
+import numpy as np
+
+from . import binding as B
+
+
+def _torch():
+    import torch
+    return torch
+
+
+class Overlap:
+    """D[mu] = 1/2 (1 + mu + (1 - mu) gamma5 sign(K)), K = gamma5 (D_W - m_w)  (eq. 2.1-2.3).
+
+    dims = (Lx, Ly, Lz, Lt); links: canonical (V,4,3,3) complex128 (numpy, CPU tensor or CUDA tensor).
+    Spinors: (V,4,3) complex128 for prec='f64', complex64 for prec='f32'.
+    """
+
+    def __init__(self, dims, links, prec="f64", recon=18, stream=None, m_w=1.5, lambda_max=6.5):
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1510_06897_b200 needs a CUDA device (no CPU fallback)")
+        self.dims = tuple(int(d) for d in dims)
+        self.V = int(np.prod(self.dims))
+        self.prec = B.OVL_F64 if prec in ("f64", B.OVL_F64) else B.OVL_F32
+        self.recon = int(recon)
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self.ctx = B.ovl_create(self.dims, links, self.prec, self.recon, self.stream.cuda_stream)
+        B.ovl_set_kernel(self.ctx, m_w, lambda_max)
+        self.cdtype = torch.complex128 if self.prec == B.OVL_F64 else torch.complex64
+
+    def close(self):
+        if getattr(self, "ctx", None) is not None:
+            B.ovl_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # ---- configuration
+    def set_chebyshev(self, alpha):
+        B.ovl_set_chebyshev(self.ctx, alpha)
+        return B.ovl_poly_orders(self.ctx)
+
+    def set_deflation(self, phi, lam):
+        B.ovl_set_deflation(self.ctx, phi, lam)
+
+    # ---- helpers
+    def _like(self, psi):
+        if isinstance(psi, np.ndarray):
+            return np.empty_like(psi)
+        return _torch().empty_like(psi)
+
+    def _run(self, fn, psi, *args):
+        out = self._like(psi)
+        fn(self.ctx, *args, psi, out)
+        return out
+
+    # ---- the path
+    def dw(self, psi):
+        return self._run(B.ovl_dw, psi)
+
+    def khat(self, psi):
+        return self._run(B.ovl_khat, psi)
+
+    def sign(self, psi):
+        return self._run(B.ovl_sign, psi)
+
+    def overlap(self, psi, mu, dagger=False):
+        return self._run(B.ovl_overlap, psi, mu, int(dagger))
+
+    def cg(self, b, mu, tol=1e-8, maxiter=1000):
+        """Solve D^dag D x = b. Returns (x, iterations, true relative residual, converged)."""
+        x = self._like(b)
+        rc, it, rel = B.ovl_cg(self.ctx, mu, b, x, tol, maxiter)
+        return x, it, rel, rc == B.OVL_OK
+
+    # ---- native-layout fields
+    def native_empty(self):
+        torch = _torch()
+        return torch.empty(B.ovl_field_bytes(self.ctx), dtype=torch.uint8, device="cuda")
+
+    def to_native(self, psi):
+        nat = self.native_empty()
+        B.ovl_field_import(self.ctx, psi, nat)
+        return nat
+
+    def from_native(self, nat, like=None):
+        torch = _torch()
+        out = torch.empty((self.V, 4, 3), dtype=self.cdtype, device="cuda") if like is None else self._like(like)
+        B.ovl_field_export(self.ctx, nat, out)
+        return out
+
+    def dw_native(self, nat_in, nat_out):
+        B.ovl_dw_native(self.ctx, nat_in, nat_out)
+
+    def overlap_native(self, nat_in, nat_out, mu, dagger=False):
+        B.ovl_overlap_native(self.ctx, mu, int(dagger), nat_in, nat_out)
+
+    # ---- measurement
+    def set_profiling(self, on=True):
+        B.ovl_set_profiling(self.ctx, on)
+
+    def last_poly_timing(self):
+        return B.ovl_last_poly_timing(self.ctx)
+
+    def launch_count(self):
+        return B.ovl_launch_count(self.ctx)

@@ -1,0 +1,200 @@
+"""Thin ctypes binding of the C-ABI in include/ovl.h -- same names, argument marshalling only.
+
+Every step of the path runs inside libovl.so's CUDA kernels.  There is no CPU fallback: if the library
+is missing or cannot be loaded, importing a symbol from it raises.  PyTorch supplies device memory and
+streams; numpy arrays are passed as host pointers (the library stages them itself).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+OVL_OK, OVL_EINVAL, OVL_ENOMEM, OVL_ECUDA, OVL_ESTATE, OVL_ENOTCONV = range(6)
+OVL_F64, OVL_F32 = 0, 1
+OVL_RECON18, OVL_RECON12 = 18, 12
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libovl.so")
+
+# name -> (restype, argtypes); mirrors include/ovl.h one to one (tests/test_abi.py checks the header against this)
+_P, _I, _D = C.c_void_p, C.c_int, C.c_double
+SIGNATURES = {
+    "ovl_version": (C.c_char_p, []),
+    "ovl_device_bytes": (C.c_size_t, [C.POINTER(_I), _I, _I, _I]),
+    "ovl_create": (_I, [C.POINTER(_P), C.POINTER(_I), _P, _I, _I, _P]),
+    "ovl_destroy": (_I, [_P]),
+    "ovl_set_kernel": (_I, [_P, _D, _D]),
+    "ovl_set_chebyshev": (_I, [_P, _I, C.POINTER(_D)]),
+    "ovl_poly_orders": (_I, [_P]),
+    "ovl_set_deflation": (_I, [_P, _I, _P, C.POINTER(_D)]),
+    "ovl_dw": (_I, [_P, _P, _P]),
+    "ovl_khat": (_I, [_P, _P, _P]),
+    "ovl_sign": (_I, [_P, _P, _P]),
+    "ovl_overlap": (_I, [_P, _D, _I, _P, _P]),
+    "ovl_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_last_error": (C.c_char_p, [_P]),
+    "ovl_field_bytes": (C.c_size_t, [_P]),
+    "ovl_field_import": (_I, [_P, _P, _P]),
+    "ovl_field_export": (_I, [_P, _P, _P]),
+    "ovl_dw_native": (_I, [_P, _P, _P]),
+    "ovl_overlap_native": (_I, [_P, _D, _I, _P, _P]),
+    "ovl_set_profiling": (_I, [_P, _I]),
+    "ovl_last_poly_timing": (_I, [_P, C.POINTER(C.c_float), C.POINTER(_I)]),
+    "ovl_launch_count": (C.c_longlong, [_P]),
+}
+
+_lib = None
+
+
+class OvlError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"ovl status {code}: {msg}")
+        self.code = code
+
+
+def load_library(path: str = LIB_PATH) -> C.CDLL:
+    """dlopen libovl.so and declare every prototype. Raises if the library is absent (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(path):
+            raise ImportError(
+                f"{path} is missing: build it with `python -m paper_1510_06897_b200.build` "
+                "(there is no CPU fallback for the overlap path)")
+        lib = C.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _ptr(a):
+    """Raw address of a torch tensor (device or CPU) or a numpy array; contiguity is the caller's contract."""
+    if isinstance(a, np.ndarray):
+        if not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("numpy arguments must be C-contiguous")
+        return C.c_void_p(a.ctypes.data)
+    if hasattr(a, "data_ptr"):
+        if not a.is_contiguous():
+            raise ValueError("tensor arguments must be contiguous")
+        return C.c_void_p(a.data_ptr())
+    if a is None:
+        return C.c_void_p(0)
+    return C.c_void_p(int(a))
+
+
+def _dbl(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(_D))
+
+
+def _check(ctx, rc, ok=(OVL_OK,)):
+    if rc not in ok:
+        msg = load_library().ovl_last_error(ctx).decode() if ctx else "no context"
+        raise OvlError(rc, msg)
+    return rc
+
+
+# ------------------------------------------------------------------ same names as the C-ABI
+
+def ovl_version() -> str:
+    return load_library().ovl_version().decode()
+
+
+def ovl_device_bytes(dims, prec=OVL_F64, recon=OVL_RECON18, max_nev=0) -> int:
+    return int(load_library().ovl_device_bytes((_I * 4)(*map(int, dims)), prec, recon, max_nev))
+
+
+def ovl_create(dims, links, prec=OVL_F64, recon=OVL_RECON18, stream=0):
+    ctx = _P()
+    rc = load_library().ovl_create(C.byref(ctx), (_I * 4)(*map(int, dims)), _ptr(links), prec, recon, _P(int(stream)))
+    if rc != OVL_OK:
+        raise OvlError(rc, "ovl_create failed")
+    return ctx
+
+
+def ovl_destroy(ctx):
+    return _check(None, load_library().ovl_destroy(ctx))
+
+
+def ovl_set_kernel(ctx, m_w=1.5, lambda_max=6.5):
+    return _check(ctx, load_library().ovl_set_kernel(ctx, m_w, lambda_max))
+
+
+def ovl_set_chebyshev(ctx, alpha):
+    a, p = _dbl(alpha)
+    return _check(ctx, load_library().ovl_set_chebyshev(ctx, len(a) - 1, p))
+
+
+def ovl_poly_orders(ctx) -> int:
+    return int(load_library().ovl_poly_orders(ctx))
+
+
+def ovl_set_deflation(ctx, phi, lam):
+    l, p = _dbl(lam)
+    return _check(ctx, load_library().ovl_set_deflation(ctx, len(l), _ptr(phi) if len(l) else _P(0), p))
+
+
+def ovl_dw(ctx, psi, out):
+    return _check(ctx, load_library().ovl_dw(ctx, _ptr(psi), _ptr(out)))
+
+
+def ovl_khat(ctx, psi, out):
+    return _check(ctx, load_library().ovl_khat(ctx, _ptr(psi), _ptr(out)))
+
+
+def ovl_sign(ctx, psi, out):
+    return _check(ctx, load_library().ovl_sign(ctx, _ptr(psi), _ptr(out)))
+
+
+def ovl_overlap(ctx, mu, dagger, psi, out):
+    return _check(ctx, load_library().ovl_overlap(ctx, float(mu), int(dagger), _ptr(psi), _ptr(out)))
+
+
+def ovl_cg(ctx, mu, b, x, tol, maxiter):
+    """Returns (status, iterations, true relative residual); status is OVL_OK or OVL_ENOTCONV."""
+    it, rel = _I(0), _D(0.0)
+    rc = load_library().ovl_cg(ctx, float(mu), _ptr(b), _ptr(x), float(tol), int(maxiter), C.byref(it), C.byref(rel))
+    _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, int(it.value), float(rel.value)
+
+
+def ovl_last_error(ctx) -> str:
+    return load_library().ovl_last_error(ctx).decode()
+
+
+def ovl_field_bytes(ctx) -> int:
+    return int(load_library().ovl_field_bytes(ctx))
+
+
+def ovl_field_import(ctx, canonical, native):
+    return _check(ctx, load_library().ovl_field_import(ctx, _ptr(canonical), _ptr(native)))
+
+
+def ovl_field_export(ctx, native, canonical):
+    return _check(ctx, load_library().ovl_field_export(ctx, _ptr(native), _ptr(canonical)))
+
+
+def ovl_dw_native(ctx, in_native, out_native):
+    return _check(ctx, load_library().ovl_dw_native(ctx, _ptr(in_native), _ptr(out_native)))
+
+
+def ovl_overlap_native(ctx, mu, dagger, in_native, out_native):
+    return _check(ctx, load_library().ovl_overlap_native(ctx, float(mu), int(dagger), _ptr(in_native), _ptr(out_native)))
+
+
+def ovl_set_profiling(ctx, on=True):
+    return _check(ctx, load_library().ovl_set_profiling(ctx, int(bool(on))))
+
+
+def ovl_last_poly_timing(ctx):
+    """(milliseconds of the last profiled polynomial loop, fused-kernel launches in it)."""
+    ms, n = C.c_float(0.0), _I(0)
+    _check(ctx, load_library().ovl_last_poly_timing(ctx, C.byref(ms), C.byref(n)))
+    return float(ms.value), int(n.value)
+
+
+def ovl_launch_count(ctx) -> int:
+    return int(load_library().ovl_launch_count(ctx))

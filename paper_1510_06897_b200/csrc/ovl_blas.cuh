@@ -1,0 +1,222 @@
+// ovl_blas.cuh -- layout import/export (a1), deflation projection / update (a5-a8), CG vector kernels (a9).
+// All reductions accumulate in fp64 with a fixed tree (thread-serial, warp shuffle, smem across warps, then a
+// single-block second stage), so results are bit-identical run to run (no float atomics).
+#pragma once
+#include "ovl_types.cuh"
+
+namespace ovl {
+
+constexpr int BLAS_THREADS = 256;
+
+// ---------------------------------------------------------------- a1: canonical AoS <-> native SoA
+// canonical spinor [V][12] complex (TS = double or float) -> native planes [12][V] of T
+template <typename TS, typename T>
+__global__ void k_import_spinor(int V, const cx<TS> *__restrict__ src, cx<T> *__restrict__ dst) {
+    const size_t n = (size_t)12 * V;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const int k = (int)(e / V);
+        const int s = (int)(e - (size_t)k * V);
+        const cx<TS> v = src[(size_t)s * 12 + k];
+        dst[e] = mk<T>((T)v.x, (T)v.y);
+    }
+}
+template <typename T, typename TD>
+__global__ void k_export_spinor(int V, const cx<T> *__restrict__ src, cx<TD> *__restrict__ dst) {
+    const size_t n = (size_t)12 * V;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const int s = (int)(e / 12);
+        const int k = (int)(e - (size_t)s * 12);
+        const cx<T> v = src[(size_t)k * V + s];
+        dst[e] = mk<TD>((TD)v.x, (TD)v.y);
+    }
+}
+// canonical links [V][4][3][3] complex128 -> native [mu][row < NROW][col][V] of T (round to nearest for fp32)
+template <typename T>
+__global__ void k_import_links(int V, int nrow, const double2 *__restrict__ src, cx<T> *__restrict__ dst) {
+    const size_t n = (size_t)4 * nrow * 3 * V;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const int pl = (int)(e / V);  // (mu*nrow + r)*3 + c
+        const int s = (int)(e - (size_t)pl * V);
+        const int c = pl % 3, r = (pl / 3) % nrow, mu = pl / (3 * nrow);
+        const double2 v = src[((size_t)s * 4 + mu) * 9 + r * 3 + c];
+        dst[e] = mk<T>((T)v.x, (T)v.y);
+    }
+}
+
+// ---------------------------------------------------------------- block reduction of NV fp64 values (fixed tree)
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+// returns the block total in thread 0 (other threads: garbage). smem: BLAS_THREADS/32 doubles.
+__device__ __forceinline__ double block_sum(double v, double *sm) {
+    v = warp_sum(v);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) sm[w] = v;
+    __syncthreads();
+    double r = 0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) r += sm[i];
+    return r;
+}
+
+// ---------------------------------------------------------------- a5: c_i = phi_i^dag psi, i < nev
+// grid = (nblk, 1); block b owns the elements [b*CH, (b+1)*CH) of the flat 12V-complex field for ALL i:
+// psi chunk held in registers, every phi_i streamed once.  partial[i*nblk + b] (complex fp64).
+constexpr int PROJ_EPT = 4;  // elements per thread
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS)
+k_project(size_t n, int nev, const cx<T> *__restrict__ phi, const cx<T> *__restrict__ psi, double2 *__restrict__ partial) {
+    __shared__ double sm[2 * (BLAS_THREADS / 32)];
+    const size_t base = (size_t)blockIdx.x * (BLAS_THREADS * PROJ_EPT) + threadIdx.x;
+    cx<T> p[PROJ_EPT];
+#pragma unroll
+    for (int j = 0; j < PROJ_EPT; ++j) {
+        const size_t e = base + (size_t)j * BLAS_THREADS;
+        p[j] = e < n ? psi[e] : mk<T>(0, 0);
+    }
+    for (int i = 0; i < nev; ++i) {
+        const cx<T> *ph = phi + (size_t)i * n;
+        double re = 0, im = 0;
+#pragma unroll
+        for (int j = 0; j < PROJ_EPT; ++j) {
+            const size_t e = base + (size_t)j * BLAS_THREADS;
+            if (e < n) {
+                const cx<T> f = ldg(ph + e);
+                re += (double)f.x * (double)p[j].x + (double)f.y * (double)p[j].y;
+                im += (double)f.x * (double)p[j].y - (double)f.y * (double)p[j].x;
+            }
+        }
+        const double r0 = block_sum(re, sm);
+        const double r1 = block_sum(im, sm + BLAS_THREADS / 32);
+        if (threadIdx.x == 0) partial[(size_t)i * gridDim.x + blockIdx.x] = make_double2(r0, r1);
+    }
+}
+// second stage: one block per i; w_i = coef_i * sum_b partial[i][b]   (a6: coef_i = sign(lambda_i) - p(lambda^_i))
+__global__ void __launch_bounds__(BLAS_THREADS)
+k_project_final(int nblk, const double2 *__restrict__ partial, const double *__restrict__ coef, double2 *__restrict__ w) {
+    __shared__ double sm[2 * (BLAS_THREADS / 32)];
+    const int i = blockIdx.x;
+    double re = 0, im = 0;
+    for (int b = threadIdx.x; b < nblk; b += blockDim.x) {
+        const double2 v = partial[(size_t)i * nblk + b];
+        re += v.x; im += v.y;
+    }
+    const double r0 = block_sum(re, sm);
+    const double r1 = block_sum(im, sm + BLAS_THREADS / 32);
+    if (threadIdx.x == 0) w[i] = make_double2(coef[i] * r0, coef[i] * r1);
+}
+
+// ---------------------------------------------------------------- a7 + a8: s = acc + sum_i w_i phi_i;  out = a psi + b [gamma5] s
+// flat element e = k*V + s: gamma5 is -1 for e >= 6V (planes of spin 2,3).
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS)
+k_deflate_assemble(size_t n, size_t n_upper, int nev, const cx<T> *__restrict__ phi, const double2 *__restrict__ w,
+                   const cx<T> *__restrict__ psi, const cx<T> *__restrict__ acc, T a, T b, int g5, cx<T> *__restrict__ out) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const cx<T> s0 = acc[e];
+    // the deflation sum is carried in fp64 and added to the polynomial part once
+    double re = 0, im = 0;
+    for (int i = 0; i < nev; ++i) {
+        const cx<T> f = ldg(phi + (size_t)i * n + e);
+        const double2 wi = w[i];
+        re += wi.x * (double)f.x - wi.y * (double)f.y;
+        im += wi.x * (double)f.y + wi.y * (double)f.x;
+    }
+    T sx = (T)((double)s0.x + re), sy = (T)((double)s0.y + im);
+    if (g5 && e >= n_upper) { sx = -sx; sy = -sy; }
+    cx<T> r;
+    if (a != T(0)) {
+        const cx<T> p = psi[e];
+        r.x = fma(a, p.x, b * sx);
+        r.y = fma(a, p.y, b * sy);
+    } else {
+        r.x = b * sx; r.y = b * sy;
+    }
+    out[e] = r;
+}
+
+// out = gamma5 in (only used to form the input of sign() in D^dag)
+template <typename T>
+__global__ void k_gamma5(size_t n, size_t n_upper, const cx<T> *__restrict__ in, cx<T> *__restrict__ out) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    cx<T> v = in[e];
+    if (e >= n_upper) { v.x = -v.x; v.y = -v.y; }
+    out[e] = v;
+}
+
+// ---------------------------------------------------------------- a9: CG vector kernels (device-side scalars)
+// sc[]: 0 rr, 1 pAp, 2 alpha, 3 beta, 4 bb
+enum { SC_RR = 0, SC_PAP = 1, SC_ALPHA = 2, SC_BETA = 3, SC_BB = 4, SC_N = 8 };
+
+// partial[b] = sum Re(conj(x) y) over the block's grid-stride elements
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS)
+k_redot(size_t n, const cx<T> *__restrict__ x, const cx<T> *__restrict__ y, double *__restrict__ partial) {
+    __shared__ double sm[BLAS_THREADS / 32];
+    double r = 0;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const cx<T> a = x[e], b = y[e];
+        r += (double)a.x * (double)b.x + (double)a.y * (double)b.y;
+    }
+    r = block_sum(r, sm);
+    if (threadIdx.x == 0) partial[blockIdx.x] = r;
+}
+// x += alpha p, r -= alpha q, partial[b] = |r|^2      (alpha = sc[SC_ALPHA])
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS)
+k_cg_update(size_t n, const double *__restrict__ sc, const cx<T> *__restrict__ p, const cx<T> *__restrict__ q,
+            cx<T> *__restrict__ x, cx<T> *__restrict__ r, double *__restrict__ partial) {
+    __shared__ double sm[BLAS_THREADS / 32];
+    const T al = (T)sc[SC_ALPHA];
+    double acc = 0;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const cx<T> pe = p[e], qe = q[e];
+        cx<T> xe = x[e], re = r[e];
+        xe.x = fma(al, pe.x, xe.x); xe.y = fma(al, pe.y, xe.y);
+        re.x = fma(-al, qe.x, re.x); re.y = fma(-al, qe.y, re.y);
+        x[e] = xe; r[e] = re;
+        acc += (double)re.x * (double)re.x + (double)re.y * (double)re.y;
+    }
+    acc = block_sum(acc, sm);
+    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+}
+// p = r + beta p   (beta = sc[SC_BETA])
+template <typename T>
+__global__ void k_xpay(size_t n, const double *__restrict__ sc, const cx<T> *__restrict__ r, cx<T> *__restrict__ p) {
+    const T be = (T)sc[SC_BETA];
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const cx<T> re = r[e];
+        cx<T> pe = p[e];
+        pe.x = fma(be, pe.x, re.x); pe.y = fma(be, pe.y, re.y);
+        p[e] = pe;
+    }
+}
+// out = x - y  (true residual)
+template <typename T>
+__global__ void k_sub(size_t n, const cx<T> *__restrict__ x, const cx<T> *__restrict__ y, cx<T> *__restrict__ out) {
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const cx<T> a = x[e], b = y[e];
+        out[e] = mk<T>(a.x - b.x, a.y - b.y);
+    }
+}
+// second stage of the CG reductions, one block.  what: 0 -> bb = rr = sum (start), 1 -> pAp = sum, alpha = rr / pAp,
+// 2 -> rr_new = sum, beta = rr_new / rr, rr = rr_new, 3 -> sc[SC_PAP] = sum (generic norm^2 read-out)
+__global__ void __launch_bounds__(BLAS_THREADS) k_cg_scalars(int nblk, const double *__restrict__ partial, double *sc, int what) {
+    __shared__ double sm[BLAS_THREADS / 32];
+    double r = 0;
+    for (int b = threadIdx.x; b < nblk; b += blockDim.x) r += partial[b];
+    r = block_sum(r, sm);
+    if (threadIdx.x == 0) {
+        if (what == 0) { sc[SC_BB] = r; sc[SC_RR] = r; }
+        else if (what == 1) { sc[SC_PAP] = r; sc[SC_ALPHA] = sc[SC_RR] / r; }
+        else if (what == 2) { sc[SC_BETA] = r / sc[SC_RR]; sc[SC_RR] = r; }
+        else { sc[SC_PAP] = r; }
+    }
+}
+
+}  // namespace ovl

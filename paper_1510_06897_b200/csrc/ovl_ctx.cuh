@@ -1,0 +1,118 @@
+// ovl_ctx.cuh -- the context behind the opaque ovl_ctx of include/ovl.h, and small host helpers.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "../../include/ovl.h"
+#include "ovl_types.cuh"
+
+struct ovl_ctx {
+    ovl::Geom g{};
+    int prec = OVL_F64, recon = OVL_RECON18;
+    cudaStream_t st = nullptr;
+    double m_w = 1.5, lambda_max = 6.5;
+
+    // eq. 2.3 inputs
+    std::vector<double> alpha;  // alpha[0..N]
+    int norders = 0;            // K^ applications actually run (last non-zero alpha, >= 1)
+    int nev = 0;
+    std::vector<double> lambda, coef;  // coef_i = sign(lambda_i) - p(lambda_i / lambda_max)
+    bool coef_stale = true;
+
+    // device memory owned by the context (all native layout unless said otherwise)
+    void *U = nullptr;    // links
+    void *phi = nullptr;  // eigenvectors [nev][12][V]
+    void *psi_n = nullptr, *out_n = nullptr, *tA = nullptr, *tB = nullptr, *acc = nullptr, *g5b = nullptr;
+    void *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr, *cg_Ap = nullptr;
+    void *stage_in = nullptr, *stage_out = nullptr;  // canonical staging for host pointers (12V complex128 each)
+    double2 *proj_partial = nullptr, *w_dev = nullptr;
+    double *coef_dev = nullptr;
+    int proj_nblk = 0, proj_cap = 0;
+    double *red_partial = nullptr, *sc_dev = nullptr, *sc_host = nullptr;
+    int red_nblk = 0;
+
+    // measurement
+    bool profiling = false;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    int last_poly_launches = 0;
+    bool poly_timed = false;
+    long long launches = 0;
+
+    char err[256] = {0};
+
+    size_t n() const { return (size_t)12 * g.V; }                       // complex elements per spinor
+    size_t tsize() const { return prec == OVL_F64 ? sizeof(double) : sizeof(float); }
+    size_t field_bytes() const { return n() * 2 * tsize(); }
+    size_t canon_bytes() const { return n() * 2 * tsize(); }            // canonical spinor at the boundary
+    int nrow() const { return recon == OVL_RECON18 ? 3 : 2; }
+    size_t link_bytes() const { return (size_t)4 * nrow() * 3 * g.V * 2 * tsize(); }
+};
+
+namespace ovl {
+
+inline int fail(ovl_ctx *c, int code, const char *fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof c->err, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define OVL_CUDA(c, call)                                                                              \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess) {                                                                       \
+            cudaGetLastError();                                                                        \
+            return ovl::fail((c), e_ == cudaErrorMemoryAllocation ? OVL_ENOMEM : OVL_ECUDA, "%s: %s", #call, \
+                             cudaGetErrorString(e_));                                                  \
+        }                                                                                              \
+    } while (0)
+
+#define OVL_TRY(expr)                  \
+    do {                               \
+        int rc_ = (expr);              \
+        if (rc_ != OVL_OK) return rc_; \
+    } while (0)
+
+// device (or managed) pointer -> usable by kernels in place; anything else is treated as host memory
+inline bool is_device_ptr(const void *p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+inline int dev_alloc(ovl_ctx *c, void **p, size_t bytes) {
+    if (*p) return OVL_OK;
+    OVL_CUDA(c, cudaMalloc(p, bytes ? bytes : 16));
+    return OVL_OK;
+}
+
+inline int grid_for(size_t n, int threads, int cap = 148 * 16) {
+    size_t b = (n + threads - 1) / threads;
+    if (b > (size_t)cap) b = cap;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+// p(x) = sum_m alpha_m T_m(x) for a real scalar (a6), Clenshaw's backward recurrence in fp64
+inline double cheb_scalar(const std::vector<double> &alpha, double x) {
+    double b1 = 0, b2 = 0;
+    for (int k = (int)alpha.size() - 1; k >= 1; --k) {
+        const double b0 = alpha[k] + 2.0 * x * b1 - b2;
+        b2 = b1;
+        b1 = b0;
+    }
+    return alpha[0] + x * b1 - b2;
+}
+
+}  // namespace ovl

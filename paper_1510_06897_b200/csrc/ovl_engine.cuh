@@ -1,0 +1,179 @@
+// ovl_engine.cuh -- host-side drivers: kernel launches for one stencil pass, the Chebyshev loop (a4),
+// deflation (a5-a7), overlap assembly (a8) and CG on D^dag D (a9).  Everything here only enqueues kernels.
+#pragma once
+#include "ovl_blas.cuh"
+#include "ovl_ctx.cuh"
+#include "ovl_wilson.cuh"
+
+namespace ovl {
+
+#define OVL_LAUNCH_CHECK(c)                                                                      \
+    do {                                                                                         \
+        ++(c)->launches;                                                                         \
+        cudaError_t e_ = cudaGetLastError();                                                     \
+        if (e_ != cudaSuccess) return fail((c), OVL_ECUDA, "kernel launch: %s", cudaGetErrorString(e_)); \
+    } while (0)
+
+template <typename T, int RECON, int FLAGS>
+inline void launch_wilson_t(ovl_ctx *c, const cx<T> *in, const cx<T> *prev, cx<T> *out, cx<T> *acc, StepParams<T> sp) {
+    const int grid = (c->g.V + WILSON_THREADS - 1) / WILSON_THREADS;
+    k_wilson_fused<T, RECON, FLAGS><<<grid, WILSON_THREADS, 0, c->st>>>(c->g, (const cx<T> *)c->U, in, prev, out, acc, sp);
+}
+
+template <typename T, int FLAGS>
+inline int launch_wilson(ovl_ctx *c, const void *in, const void *prev, void *out, void *acc, double c_diag, double c_hop,
+                         double a0, double a1) {
+    StepParams<T> sp{(T)c_diag, (T)c_hop, (T)a0, (T)a1};
+    if (c->recon == OVL_RECON18)
+        launch_wilson_t<T, 18, FLAGS>(c, (const cx<T> *)in, (const cx<T> *)prev, (cx<T> *)out, (cx<T> *)acc, sp);
+    else
+        launch_wilson_t<T, 12, FLAGS>(c, (const cx<T> *)in, (const cx<T> *)prev, (cx<T> *)out, (cx<T> *)acc, sp);
+    OVL_LAUNCH_CHECK(c);
+    return OVL_OK;
+}
+
+// out = D_W in
+template <typename T> int dw_native(ovl_ctx *c, const void *in, void *out) {
+    return launch_wilson<T, F_WRITE>(c, in, nullptr, out, nullptr, 4.0, -0.5, 0, 0);
+}
+// out = K^ in
+template <typename T> int khat_native(ovl_ctx *c, const void *in, void *out) {
+    return launch_wilson<T, F_G5 | F_WRITE>(c, in, nullptr, out, nullptr, (4.0 - c->m_w) / c->lambda_max,
+                                            -0.5 / c->lambda_max, 0, 0);
+}
+
+// acc = sum_{m=0}^{norders} alpha_m T_m(K^) src    (first sum of eq. 2.3; src is not modified)
+template <typename T> int cheb_native(ovl_ctx *c, const void *src) {
+    const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
+    const std::vector<double> &al = c->alpha;
+    const int N = c->norders;
+    if (c->profiling) OVL_CUDA(c, cudaEventRecord(c->ev0, c->st));
+    if (N == 1)
+        OVL_TRY((launch_wilson<T, F_G5 | F_ACC_INIT>(c, src, nullptr, nullptr, c->acc, cd, ch, al[0], al[1])));
+    else
+        OVL_TRY((launch_wilson<T, F_G5 | F_WRITE | F_ACC_INIT>(c, src, nullptr, c->tA, c->acc, cd, ch, al[0], al[1])));
+    for (int m = 1; m < N; ++m) {  // produces t_{m+1}
+        const void *in = (m & 1) ? c->tA : c->tB;
+        void *out = (m & 1) ? c->tB : c->tA;
+        const void *prev = (m == 1) ? src : out;
+        const double a1 = al[m + 1];
+        const bool last = (m + 1 == N);
+        if (last)
+            OVL_TRY((launch_wilson<T, F_G5 | F_PREV | F_ACC_ADD>(c, in, prev, nullptr, c->acc, 2 * cd, 2 * ch, 0, a1)));
+        else if (a1 != 0.0)
+            OVL_TRY((launch_wilson<T, F_G5 | F_PREV | F_WRITE | F_ACC_ADD>(c, in, prev, out, c->acc, 2 * cd, 2 * ch, 0, a1)));
+        else
+            OVL_TRY((launch_wilson<T, F_G5 | F_PREV | F_WRITE>(c, in, prev, out, nullptr, 2 * cd, 2 * ch, 0, 0)));
+    }
+    if (c->profiling) {
+        OVL_CUDA(c, cudaEventRecord(c->ev1, c->st));
+        c->last_poly_launches = N;
+        c->poly_timed = true;
+    }
+    return OVL_OK;
+}
+
+inline int refresh_coef(ovl_ctx *c) {
+    if (!c->coef_stale || c->nev == 0) return OVL_OK;
+    c->coef.resize(c->nev);
+    for (int i = 0; i < c->nev; ++i) {
+        const double l = c->lambda[i];
+        const double sg = (l > 0) - (l < 0);
+        c->coef[i] = sg - cheb_scalar(c->alpha, l / c->lambda_max);
+    }
+    OVL_CUDA(c, cudaMemcpyAsync(c->coef_dev, c->coef.data(), sizeof(double) * c->nev, cudaMemcpyHostToDevice, c->st));
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));  // coef.data() is pageable host memory
+    c->coef_stale = false;
+    return OVL_OK;
+}
+
+// out = a*in + b*[gamma5]( sign(K) src ),  src = in (dagger = 0) or gamma5 in (dagger = 1, gamma5 not applied on the way out)
+// a = b = ... chosen by the caller: ovl_sign uses a = 0, b = 1, g5out = 0.
+template <typename T> int sign_combine_native(ovl_ctx *c, double a, double b, int dagger, int g5out, const void *in, void *out) {
+    if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
+    const size_t n = c->n(), n_upper = (size_t)6 * c->g.V;
+    const void *src = in;
+    if (dagger) {
+        k_gamma5<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(n, n_upper, (const cx<T> *)in, (cx<T> *)c->g5b);
+        OVL_LAUNCH_CHECK(c);
+        src = c->g5b;
+    }
+    if (c->nev > 0) {
+        OVL_TRY(refresh_coef(c));
+        k_project<T><<<c->proj_nblk, BLAS_THREADS, 0, c->st>>>(n, c->nev, (const cx<T> *)c->phi, (const cx<T> *)src, c->proj_partial);
+        OVL_LAUNCH_CHECK(c);
+        k_project_final<<<c->nev, BLAS_THREADS, 0, c->st>>>(c->proj_nblk, c->proj_partial, c->coef_dev, c->w_dev);
+        OVL_LAUNCH_CHECK(c);
+    }
+    OVL_TRY(cheb_native<T>(c, src));
+    k_deflate_assemble<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(
+        n, n_upper, c->nev, (const cx<T> *)c->phi, c->w_dev, (const cx<T> *)in, (const cx<T> *)c->acc, (T)a, (T)b, g5out,
+        (cx<T> *)out);
+    OVL_LAUNCH_CHECK(c);
+    return OVL_OK;
+}
+
+template <typename T> int overlap_native(ovl_ctx *c, double mu, int dagger, const void *in, void *out) {
+    return sign_combine_native<T>(c, 0.5 * (1.0 + mu), 0.5 * (1.0 - mu), dagger, dagger ? 0 : 1, in, out);
+}
+
+// ---- CG on A = D^dag D (a9).  b_n, x_n native; x0 = 0.
+template <typename T> int reduce_redot(ovl_ctx *c, const void *x, const void *y, int what) {
+    k_redot<T><<<c->red_nblk, BLAS_THREADS, 0, c->st>>>(c->n(), (const cx<T> *)x, (const cx<T> *)y, c->red_partial);
+    OVL_LAUNCH_CHECK(c);
+    k_cg_scalars<<<1, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, what);
+    OVL_LAUNCH_CHECK(c);
+    return OVL_OK;
+}
+inline int fetch_scalars(ovl_ctx *c) {
+    OVL_CUDA(c, cudaMemcpyAsync(c->sc_host, c->sc_dev, sizeof(double) * SC_N, cudaMemcpyDeviceToHost, c->st));
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    return OVL_OK;
+}
+
+template <typename T>
+int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int maxiter, int *iters, double *relres) {
+    const size_t n = c->n(), fb = c->field_bytes();
+    OVL_TRY(dev_alloc(c, &c->cg_r, fb));
+    OVL_TRY(dev_alloc(c, &c->cg_p, fb));
+    OVL_TRY(dev_alloc(c, &c->cg_q, fb));
+    OVL_TRY(dev_alloc(c, &c->cg_Ap, fb));
+    OVL_CUDA(c, cudaMemsetAsync(x_n, 0, fb, c->st));
+    OVL_CUDA(c, cudaMemcpyAsync(c->cg_r, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
+    OVL_CUDA(c, cudaMemcpyAsync(c->cg_p, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
+    OVL_TRY(reduce_redot<T>(c, b_n, b_n, 0));
+    OVL_TRY(fetch_scalars(c));
+    const double bb = c->sc_host[SC_BB];
+    double rr = bb;
+    int it = 0;
+    const int gridv = grid_for(n, BLAS_THREADS);
+    while (it < maxiter && !(tol > 0 && std::sqrt(rr) <= tol * std::sqrt(bb))) {
+        OVL_TRY(overlap_native<T>(c, mu, 0, c->cg_p, c->cg_q));
+        OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap));
+        OVL_TRY(reduce_redot<T>(c, c->cg_p, c->cg_Ap, 1));  // alpha = rr / Re(p^dag A p)
+        k_cg_update<T><<<c->red_nblk, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_p, (const cx<T> *)c->cg_Ap,
+                                                               (cx<T> *)x_n, (cx<T> *)c->cg_r, c->red_partial);
+        OVL_LAUNCH_CHECK(c);
+        k_cg_scalars<<<1, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, 2);  // beta, rr
+        OVL_LAUNCH_CHECK(c);
+        k_xpay<T><<<gridv, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_r, (cx<T> *)c->cg_p);
+        OVL_LAUNCH_CHECK(c);
+        OVL_TRY(fetch_scalars(c));  // the convergence scalar is the only host round trip per iteration
+        rr = c->sc_host[SC_RR];
+        ++it;
+        if (!(rr == rr)) return fail(c, OVL_ECUDA, "CG broke down (NaN residual) at iteration %d", it);
+    }
+    // true residual ||b - A x|| / ||b||
+    OVL_TRY(overlap_native<T>(c, mu, 0, x_n, c->cg_q));
+    OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap));
+    k_sub<T><<<gridv, BLAS_THREADS, 0, c->st>>>(n, (const cx<T> *)b_n, (const cx<T> *)c->cg_Ap, (cx<T> *)c->cg_q);
+    OVL_LAUNCH_CHECK(c);
+    OVL_TRY(reduce_redot<T>(c, c->cg_q, c->cg_q, 3));
+    OVL_TRY(fetch_scalars(c));
+    *iters = it;
+    *relres = std::sqrt(c->sc_host[SC_PAP] / bb);
+    if (tol > 0 && !(std::sqrt(rr) <= tol * std::sqrt(bb))) return fail(c, OVL_ENOTCONV, "CG: %d iterations, ||r||/||b|| = %.3e > tol", it, std::sqrt(rr / bb));
+    return OVL_OK;
+}
+
+}  // namespace ovl

@@ -1,0 +1,54 @@
+// ovl_types.cuh -- complex helpers, lattice geometry and the native (SoA, site-coalesced) field layout.
+//
+// Native layout (north_star (a)):
+//   spinor:  12 planes of V complex, plane k = 3*spin + colour:   f[k*V + s]
+//   links:   4 directions x NROW*3 planes of V complex (NROW = 3 for 18-real, 2 for 12-real storage):
+//            U[((mu*NROW + row)*3 + col)*V + s]
+// so a warp of consecutive sites reads one contiguous 512 B (fp64) / 256 B (fp32) segment per plane.
+// This file shares nothing with oracle/ (AoS, explicit 4x4 gamma matrices).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ovl {
+
+template <typename T> struct cx_of;
+template <> struct cx_of<double> { using type = double2; };
+template <> struct cx_of<float> { using type = float2; };
+template <typename T> using cx = typename cx_of<T>::type;
+
+template <typename T> __host__ __device__ __forceinline__ cx<T> mk(T re, T im) {
+    cx<T> r; r.x = re; r.y = im; return r;
+}
+// a + b, a - b
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { a.x += b.x; a.y += b.y; return a; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
+// a + i b, a - i b
+template <typename C> __device__ __forceinline__ C caddi(C a, C b) { a.x -= b.y; a.y += b.x; return a; }
+template <typename C> __device__ __forceinline__ C csubi(C a, C b) { a.x += b.y; a.y -= b.x; return a; }
+// acc += a * b
+template <typename C> __device__ __forceinline__ void cfma(C &acc, C a, C b) {
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
+}
+// acc += conj(a) * b
+template <typename C> __device__ __forceinline__ void cfmac(C &acc, C a, C b) {
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(-a.y, b.x, acc.y);
+}
+// a * b, conj(a * b)
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
+    C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+
+struct Geom {
+    int L[4];      // Lx, Ly, Lz, Lt
+    int V;         // sites
+    int sxy, sxyz; // Lx*Ly, Lx*Ly*Lz
+};
+
+// read-only (non-coherent) loads: fields are never written by the kernel that stencil-reads them
+__device__ __forceinline__ double2 ldg(const double2 *p) { return __ldg(p); }
+__device__ __forceinline__ float2 ldg(const float2 *p) { return __ldg(p); }
+
+}  // namespace ovl

@@ -213,3 +213,18 @@ def orthonormal_vectors(dims, nvec: int, seed: int) -> np.ndarray:
     a = _complex_gaussian(_rng(seed), (12 * v, nvec))
     q, _ = np.linalg.qr(a)
     return np.ascontiguousarray(q.T.reshape(nvec, v, 4, 3))
+
+
+def phase_vectors(dims, nvec: int, seed: int) -> np.ndarray:
+    """nvec exactly orthonormal vectors in O(12V) work each, for deflation-shaped inputs at volumes where a QR of a
+    (12V x nvec) Gaussian block is too expensive: phi_i[e] = exp(i (theta_e + 2 pi i e / n)) / sqrt(n), theta seeded
+    uniform phases, e the flat (site, spin, colour) index, n = 12V.  <phi_i, phi_j> = (1/n) sum_e exp(2 pi i (j-i) e/n)
+    = delta_ij.  NOT eigenvectors (reading R10).  Shape (nvec, V, 4, 3)."""
+    n = 12 * volume(dims)
+    theta = _rng(seed).uniform(0.0, 2.0 * np.pi, n)
+    e = np.arange(n, dtype=np.float64)
+    out = np.empty((nvec, n), dtype=np.complex128)
+    for i in range(nvec):
+        ang = theta + (2.0 * np.pi * i / n) * e
+        out[i] = (np.cos(ang) + 1j * np.sin(ang)) / np.sqrt(n)
+    return out.reshape(nvec, volume(dims), 4, 3)

@@ -1,0 +1,298 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element on the same
+seeded inputs.  Tolerances are BASELINE.json north_star's: 1e-12 (fp64 D_W), 1e-10 (fp64 sign / overlap /
+fixed-iteration CG), 1e-5 (fp32), relative L2 over the whole field."""
+import numpy as np
+import pytest
+
+from paper_1510_06897_b200 import inputs
+from tests.conftest import rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_DW, TOL_OVL, TOL_F32 = 1e-12, 1e-10, 1e-5
+G5 = np.array([1.0, 1.0, -1.0, -1.0])
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def api(torch):
+    from paper_1510_06897_b200 import api, binding
+    binding.load_library()  # fail loudly if the CUDA extension is missing
+    return api
+
+
+def dev(torch, a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    return t.to(dtype) if dtype is not None else t
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def rough_alpha(n, seed=5):
+    """A generic (not sign-like) table with non-zero even AND odd entries: exercises every accumulate branch."""
+    rng = np.random.default_rng(seed)
+    a = rng.standard_normal(n + 1) / (1 + np.arange(n + 1))
+    if n >= 5:
+        a[4] = 0.0
+    return a
+
+
+DW_DIMS = [(4, 4, 4, 4), (2, 2, 2, 2), (4, 6, 8, 10), (6, 4, 2, 8), (8, 8, 8, 8), (10, 6, 4, 12), (8, 8, 8, 32)]
+
+
+@pytest.mark.parametrize("dims", DW_DIMS)
+@pytest.mark.parametrize("recon", [18, 12])
+def test_dw_fp64(torch, api, orc, dims, recon):
+    U = inputs.random_links(dims, 0.7, 100 + sum(dims))
+    psi = inputs.gaussian_spinor(dims, 200 + sum(dims))
+    want = orc.dw(dims, U, psi)
+    with api.Overlap(dims, dev(torch, U), "f64", recon) as op:
+        got = host(op.dw(dev(torch, psi)))
+    assert rel_err(got, want) < TOL_DW
+    assert np.abs(got - want).max() < 1e-12 * np.abs(want).max() * 10
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (8, 8, 8, 32)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_dw_fp32(torch, api, orc, dims, recon):
+    U = inputs.random_links(dims, 0.7, 31)
+    psi = inputs.gaussian_spinor(dims, 32)
+    want = orc.dw(dims, U, psi)
+    with api.Overlap(dims, dev(torch, U), "f32", recon) as op:
+        got = host(op.dw(dev(torch, psi, torch.complex64)))
+    assert got.dtype == np.complex64
+    assert rel_err(got.astype(np.complex128), want) < TOL_F32
+
+
+def test_khat_fp64(torch, api, orc):
+    dims = (4, 6, 8, 10)
+    U = inputs.random_links(dims, 0.3, 1)
+    psi = inputs.gaussian_spinor(dims, 2)
+    with api.Overlap(dims, dev(torch, U), m_w=1.4, lambda_max=6.1) as op:
+        got = host(op.khat(dev(torch, psi)))
+    assert rel_err(got, orc.khat(dims, U, psi, 1.4, 6.1)) < TOL_DW
+
+
+@pytest.mark.parametrize("dims,N", [((4, 4, 4, 4), 1), ((4, 4, 4, 4), 2), ((4, 4, 4, 4), 3), ((4, 6, 8, 10), 24), ((6, 4, 2, 8), 37)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_sign_generic_coefficients(torch, api, orc, dims, N, recon):
+    """Every order accumulates (even and odd alpha non-zero, one zero in the middle): recurrence indexing."""
+    U = inputs.random_links(dims, 0.5, 9)
+    psi = inputs.gaussian_spinor(dims, 10)
+    alpha = rough_alpha(N)
+    want = orc.sign(dims, U, alpha, psi)
+    with api.Overlap(dims, dev(torch, U), "f64", recon) as op:
+        assert op.set_chebyshev(alpha) == N
+        got = host(op.sign(dev(torch, psi)))
+    assert rel_err(got, want) < TOL_OVL
+
+
+def test_trailing_zero_coefficients_are_skipped(torch, api, orc):
+    dims = (4, 4, 4, 4)
+    U = inputs.random_links(dims, 0.5, 9)
+    psi = inputs.gaussian_spinor(dims, 10)
+    alpha = np.concatenate([rough_alpha(9), np.zeros(5)])
+    with api.Overlap(dims, dev(torch, U)) as op:
+        assert op.set_chebyshev(alpha) == 9  # reading R7
+        got = host(op.sign(dev(torch, psi)))
+    assert rel_err(got, orc.sign(dims, U, alpha, psi)) < TOL_OVL
+
+
+def test_config0_overlap_4x4(torch, api, orc, dense44):
+    """BASELINE config 0: 4^4, U = exp(0.3 i H), D_W and D[0.1] with degree 101, no deflation; Tier A vs the oracle
+    and Tier B vs the dense exact sign function (error bounded by the polynomial's error on the spectrum)."""
+    d = dense44
+    dims, U = d["dims"], d["U"]
+    psi = inputs.gaussian_spinor(dims, inputs.SEED_BASE + 100)
+    eps = 0.95 * np.abs(d["lam"]).min() / 6.5
+    alpha = inputs.chebyshev_sign_coeffs(101, eps)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        assert op.set_chebyshev(alpha) == 101
+        p = dev(torch, psi)
+        assert rel_err(host(op.dw(p)), orc.dw(dims, U, psi)) < TOL_DW
+        got = host(op.overlap(p, 0.1))
+        got_d = host(op.overlap(p, 0.1, dagger=True))
+        s = host(op.sign(p))
+    assert rel_err(got, orc.overlap(dims, U, alpha, 0.1, psi)) < TOL_OVL
+    assert rel_err(got_d, orc.overlap(dims, U, alpha, 0.1, psi, dagger=True)) < TOL_OVL
+    delta = np.abs(inputs.chebyshev_eval(alpha, d["lam"] / 6.5) - np.sign(d["lam"])).max()
+    exact = d["S"] @ psi.ravel()
+    assert np.linalg.norm(s.ravel() - exact) / np.linalg.norm(psi) <= delta * (1 + 1e-6) + 1e-12
+    n = d["K"].shape[0]
+    g5m = np.tile(np.repeat(G5, 3), n // 12)
+    dex = 0.5 * (1.1 * psi.ravel() + 0.9 * g5m * exact)
+    assert np.linalg.norm(got.ravel() - dex) / np.linalg.norm(dex) < 2 * delta
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", TOL_OVL), ("f32", TOL_F32)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_deflated_sign_and_overlap(torch, api, orc, prec, tol, recon):
+    """eq. 2.3 complete, with generic orthonormal vectors and 'eigenvalues' of both signs (reading R10: a well-defined
+    linear map for any (phi_i, lambda_i)); coarse polynomial so the deflation term is O(1)."""
+    dims = (4, 6, 8, 10)
+    nev = 7
+    U = inputs.config_links(dims, 0.3, 3, stout_steps=1)
+    psi = inputs.gaussian_spinor(dims, 4)
+    phi = inputs.orthonormal_vectors(dims, nev, 5)
+    lam = np.array([0.31, -0.33, 0.35, -0.4, 0.42, 0.5, -0.55])
+    alpha = inputs.chebyshev_sign_coeffs(31, 0.2)
+    want_s = orc.sign(dims, U, alpha, psi, phi, lam)
+    plain = orc.sign(dims, U, alpha, psi)
+    assert rel_err(want_s, plain) > 1e-3  # deflation does something here
+    cd = torch.complex128 if prec == "f64" else torch.complex64
+    with api.Overlap(dims, dev(torch, U), prec, recon) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        p = dev(torch, psi, cd)
+        assert rel_err(host(op.sign(p)), want_s) < tol
+        for mu, dag in [(0.01, False), (0.05, True)]:
+            want = orc.overlap(dims, U, alpha, mu, psi, phi, lam, dagger=dag)
+            assert rel_err(host(op.overlap(p, mu, dagger=dag)), want) < tol
+        op.set_deflation(None, [])  # switch deflation off again
+        assert rel_err(host(op.sign(p)), plain) < tol
+
+
+def test_config1_shape_8x8x8x32_degree200_nev20(torch, api, orc):
+    """BASELINE config 1 shape: 8^3 x 32, smeared links, mu = 0.01, degree 200, 20 deflation vectors (generic
+    orthonormal stand-ins for the Lanczos vectors, DESIGN.md input recipe); several tiles + ragged last block."""
+    dims = (8, 8, 8, 32)
+    U = inputs.config_links(dims, 0.3, inputs.SEED_BASE + 1, stout_steps=3)
+    psi = inputs.gaussian_spinor(dims, inputs.SEED_BASE + 101)
+    phi = inputs.orthonormal_vectors(dims, 20, inputs.SEED_BASE + 201)
+    lam = 0.505 * np.where(np.arange(20) % 2 == 0, 1.0, -1.0) * (1 + 0.001 * np.arange(20))
+    alpha = inputs.chebyshev_sign_coeffs(200, 0.95 * 0.505 / 6.5)
+    want = orc.overlap(dims, U, alpha, 0.01, psi, phi, lam)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        assert op.set_chebyshev(alpha) == 199  # degree 200 table, alpha_200 = 0 (reading R7)
+        op.set_deflation(dev(torch, phi), lam)
+        p = dev(torch, psi)
+        got = host(op.overlap(p, 0.01))
+        s = op.sign(p)
+        s2 = host(op.sign(s))
+    assert rel_err(got, want) < TOL_OVL
+    # sign^2 = 1 up to the polynomial error (the vectors are not eigenvectors, so only the undeflated bound applies
+    # on the complement; keep it loose)
+    assert np.isfinite(s2).all()
+
+
+def test_cg_fixed_iterations_and_to_tolerance(torch, api, orc, dense44):
+    d = dense44
+    dims, U = d["dims"], d["U"]
+    mu = 0.05
+    alpha = inputs.chebyshev_sign_coeffs(101, 0.95 * np.abs(d["lam"]).min() / 6.5)
+    b = inputs.gaussian_spinor(dims, 91)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        bd = dev(torch, b)
+        # (iii) of reading R14: fixed iteration count, no stopping test
+        xk, itk, _, ok = op.cg(bd, mu, tol=0.0, maxiter=10)
+        want_k, it_o, _ = orc.cg(dims, U, alpha, mu, b, 0.0, 10)
+        assert itk == it_o == 10 and ok
+        assert rel_err(host(xk), want_k) < TOL_OVL
+        # (i) + (ii): to tolerance
+        x, it, rel, ok = op.cg(bd, mu, tol=1e-8, maxiter=500)
+        xo, ito, relo = orc.cg(dims, U, alpha, mu, b, 1e-8, 500)
+        assert ok and abs(it - ito) <= 2
+        assert rel < 1.05e-8 and relo < 1.05e-8
+        assert rel_err(host(x), xo) < 1e-5
+        # not converged -> OVL_ENOTCONV surfaced as ok = False, x = last iterate
+        x3, it3, rel3, ok3 = op.cg(bd, mu, tol=1e-8, maxiter=3)
+        assert it3 == 3 and not ok3 and rel3 > 1e-8
+        want3, _, _ = orc.cg(dims, U, alpha, mu, b, 1e-8, 3)
+        assert rel_err(host(x3), want3) < TOL_OVL
+
+
+def test_cg_with_deflation_8x8x8x8(torch, api, orc):
+    dims = (8, 8, 8, 8)
+    U = inputs.config_links(dims, 0.3, 13, stout_steps=2)
+    b = inputs.gaussian_spinor(dims, 14)
+    phi = inputs.orthonormal_vectors(dims, 5, 15)
+    lam = np.array([0.5, -0.51, 0.52, -0.53, 0.54])
+    alpha = inputs.chebyshev_sign_coeffs(61, 0.075)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        x, it, rel, ok = op.cg(dev(torch, b), 0.2, tol=0.0, maxiter=6)
+    want, _, relo = orc.cg(dims, U, alpha, 0.2, b, 0.0, 6, phi, lam)
+    assert rel_err(host(x), want) < TOL_OVL
+    assert abs(rel - relo) < 1e-9
+
+
+def test_host_pointers_and_native_fields(torch, api, orc):
+    """numpy (host) in/out through the C-ABI staging path; native import/export is an exact round trip."""
+    dims = (4, 6, 8, 10)
+    U = inputs.random_links(dims, 0.4, 51)
+    psi = inputs.gaussian_spinor(dims, 52)
+    alpha = rough_alpha(12)
+    with api.Overlap(dims, U) as op:  # host links
+        op.set_chebyshev(alpha)
+        got = op.overlap(psi, 0.1)  # host spinor in, host spinor out
+        assert isinstance(got, np.ndarray)
+        assert rel_err(got, orc.overlap(dims, U, alpha, 0.1, psi)) < TOL_OVL
+        nat = op.to_native(dev(torch, psi))
+        back = host(op.from_native(nat))
+        assert np.array_equal(back, psi)
+        nat_out = op.native_empty()
+        op.dw_native(nat, nat_out)
+        assert rel_err(host(op.from_native(nat_out)), orc.dw(dims, U, psi)) < TOL_DW
+        op.overlap_native(nat, nat_out, 0.1)
+        assert np.array_equal(host(op.from_native(nat_out)), got)
+        phi = inputs.orthonormal_vectors(dims, 3, 53)
+        lam = [0.4, -0.5, 0.6]
+        op.set_deflation(phi, lam)  # host eigenvectors
+        assert rel_err(op.sign(psi), orc.sign(dims, U, alpha, psi, phi, lam)) < TOL_OVL
+
+
+def test_bit_identical_run_to_run(torch, api):
+    dims = (6, 6, 6, 10)
+    U = dev(torch, inputs.random_links(dims, 0.4, 61))
+    psi = dev(torch, inputs.gaussian_spinor(dims, 62))
+    phi = dev(torch, inputs.orthonormal_vectors(dims, 4, 63))
+    alpha = inputs.chebyshev_sign_coeffs(41, 0.1)
+    outs = []
+    for _ in range(2):
+        with api.Overlap(dims, U) as op:
+            op.set_chebyshev(alpha)
+            op.set_deflation(phi, [0.3, -0.3, 0.4, -0.4])
+            y = op.overlap(psi, 0.03)
+            x, it, rel, _ = op.cg(psi, 0.3, tol=1e-6, maxiter=50)
+            outs.append((host(y), host(x), it, rel))
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert np.array_equal(outs[0][1], outs[1][1])
+    assert outs[0][2:] == outs[1][2:]
+
+
+def test_error_statuses(torch, api):
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 4, 4)
+    U = dev(torch, inputs.unit_links(dims))
+    psi = dev(torch, inputs.gaussian_spinor(dims, 1))
+    with pytest.raises(B.OvlError) as e:
+        api.Overlap((4, 4, 1, 4), U)
+    assert e.value.code == B.OVL_EINVAL
+    with api.Overlap(dims, U) as op:
+        with pytest.raises(B.OvlError) as e:
+            op.sign(psi)  # no polynomial yet
+        assert e.value.code == B.OVL_ESTATE and "chebyshev" in str(e.value)
+        with pytest.raises(B.OvlError) as e:
+            B.ovl_dw(op.ctx, psi, psi)  # aliasing
+        assert e.value.code == B.OVL_EINVAL
+        with pytest.raises(B.OvlError) as e:
+            op.set_chebyshev([0.0, float("nan")])
+        assert e.value.code == B.OVL_EINVAL
+        op.set_chebyshev([0.0, 1.0])
+        with pytest.raises(B.OvlError) as e:
+            op.set_deflation(psi.reshape(1, -1, 4, 3), [0.0])  # reading R9
+        assert e.value.code == B.OVL_EINVAL
+        with pytest.raises(B.OvlError) as e:
+            B.ovl_set_kernel(op.ctx, 1.5, -1.0)
+        assert e.value.code == B.OVL_EINVAL
+        assert op.launch_count() > 0
