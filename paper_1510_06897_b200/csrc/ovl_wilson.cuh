@@ -6,7 +6,9 @@
 //                                                          K^ : (4 - m_w)/lambda_max, -1/(2 lambda_max); x2 for m >= 1)
 //     w      = gamma5 w                     [F_G5]        (K = gamma5 (D_W - m_w); sign flip of spins 2,3)
 //     w     -= prev(x)                      [F_PREV]      (t_{m+1} = 2 K^ t_m - t_{m-1})
-//     out(x) = w                            [F_WRITE]     (may alias prev: same thread reads then writes site x)
+//     out(x) = w                            [F_WRITE]     (may alias prev: the ONLY aliasing pair is prev[k,x] / out[k,x], read then
+//                                                          written by the same thread with a true data dependency, so declaring
+//                                                          both __restrict__ is safe and lets the loads be batched before the stores)
 //     acc(x) = a0 * in(x) + a1 * w          [F_ACC_INIT]  (alpha_0 t_0 + alpha_1 t_1)
 //     acc(x)+= a1 * w                       [F_ACC_ADD]   (alpha_{m+1} t_{m+1})
 // This is the paper's "merging together the Wilson matrix and polynomial algebra ... into a single GPU kernel"
@@ -136,7 +138,8 @@ constexpr int WILSON_THREADS = 128;
 
 template <typename T, int RECON, int FLAGS>
 __global__ void __launch_bounds__(WILSON_THREADS)
-k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *prev, cx<T> *out,
+k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *__restrict__ prev,
+               cx<T> *__restrict__ out,
                cx<T> *__restrict__ acc, const StepParams<T> sp) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= g.V) return;

@@ -1,0 +1,89 @@
+"""GPU parity at BASELINE.json's full size (20^3 x 64, the launch configuration bench.py times): the whole D_W field
+and a low-degree deflated overlap apply against the oracle, and the degree-400 sign function against the FFT closed
+form on a pure gauge (tests/closed_forms.py), in fp64 and fp32."""
+import numpy as np
+import pytest
+
+from paper_1510_06897_b200 import inputs
+from tests.closed_forms import free_sign_fft, golden_gammas
+from tests.conftest import rel_err
+
+pytestmark = pytest.mark.gpu
+DIMS = (20, 20, 20, 64)
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def api(torch):
+    from paper_1510_06897_b200 import api, binding
+    binding.load_library()
+    return api
+
+
+@pytest.fixture(scope="module")
+def rough(torch):
+    U = inputs.random_links(DIMS, 0.25, inputs.SEED_BASE + 3)
+    psi = inputs.gaussian_spinor(DIMS, inputs.SEED_BASE + 103)
+    return U, psi
+
+
+def dev(torch, a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    return t.to(dtype) if dtype is not None else t
+
+
+@pytest.mark.parametrize("prec,recon,tol", [("f64", 18, 1e-12), ("f64", 12, 1e-12), ("f32", 18, 1e-5), ("f32", 12, 1e-5)])
+def test_dw_full_field_20x20x20x64(torch, api, orc, rough, prec, recon, tol):
+    U, psi = rough
+    want = orc.dw(DIMS, U, psi)
+    with api.Overlap(DIMS, dev(torch, U), prec, recon) as op:
+        got = op.dw(dev(torch, psi, op.cdtype)).cpu().numpy().astype(np.complex128)
+    assert rel_err(got, want) < tol
+    # sampled sites, element by element (max norm), including both t boundaries
+    v = want.shape[0]
+    sites = np.concatenate([np.arange(0, 50), np.arange(v - 50, v), np.random.default_rng(1).integers(0, v, 500)])
+    scale = np.abs(want).max()
+    assert np.abs(got[sites] - want[sites]).max() < 20 * tol * scale
+
+
+def test_low_degree_deflated_overlap_vs_oracle_full_size(torch, api, orc, rough):
+    """The fused Chebyshev step, deflation and assembly in the full-size launch configuration against the oracle
+    (degree 9 keeps the oracle to seconds; every kernel variant of the degree-400 path is exercised)."""
+    U, psi = rough
+    phi = inputs.phase_vectors(DIMS, 3, inputs.SEED_BASE + 203)
+    lam = np.array([0.5, -0.51, 0.52])
+    alpha = inputs.chebyshev_sign_coeffs(9, 0.3)
+    want = orc.overlap(DIMS, U, alpha, 0.01, psi, phi, lam)
+    with api.Overlap(DIMS, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        got = op.overlap(dev(torch, psi), 0.01).cpu().numpy()
+    assert rel_err(got, want) < 1e-10
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_degree400_sign_vs_fft_closed_form_full_size(torch, api, prec, tol):
+    """Pure gauge U_mu(x) = g(x) g(x+mu)^dag at 20^3 x 64: sign(K) psi is known in closed form at any volume. With the
+    degree-400 table the polynomial error on the spectrum is < 1e-12, so GPU vs closed form tests the whole
+    399-order recurrence in bench.py's configuration."""
+    U, g = inputs.pure_gauge_links(DIMS, inputs.SEED_BASE + 33)
+    psi = inputs.gaussian_spinor(DIMS, inputs.SEED_BASE + 133)
+    exact, omega = free_sign_fft(DIMS, psi, golden_gammas(), 1.5, g)
+    eps = 0.95 * omega.min() / 6.5
+    alpha = inputs.chebyshev_sign_coeffs(400, eps)
+    delta = np.abs(inputs.chebyshev_eval(alpha, omega.ravel() / 6.5) - 1.0).max()
+    assert delta < 1e-11
+    with api.Overlap(DIMS, dev(torch, U), prec) as op:
+        assert op.set_chebyshev(alpha) == 399
+        p = dev(torch, psi, op.cdtype)
+        s = op.sign(p)
+        got = s.cpu().numpy().astype(np.complex128)
+        s2 = op.sign(s).cpu().numpy().astype(np.complex128)
+    assert rel_err(got, exact) < tol
+    assert rel_err(s2, psi) < 2 * tol  # sign(K)^2 = 1

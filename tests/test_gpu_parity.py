@@ -296,3 +296,28 @@ def test_error_statuses(torch, api):
             B.ovl_set_kernel(op.ctx, 1.5, -1.0)
         assert e.value.code == B.OVL_EINVAL
         assert op.launch_count() > 0
+
+
+def test_deflation_exact_eigenpairs_4x4(torch, api, orc, dense44):
+    """True eigenpairs (dense 4^4): the deflated GPU map equals W diag(sign lam_i [deflated] | p(lam_i)) W^dag psi and
+    sits closer to the exact sign function than the undeflated one (coarse N = 15 polynomial)."""
+    d = dense44
+    nev = 20
+    idx = np.argsort(np.abs(d["lam"]))[:nev]
+    lam_d = d["lam"][idx]
+    phi = np.ascontiguousarray(d["W"][:, idx].T).reshape(nev, -1, 4, 3)
+    alpha = inputs.chebyshev_sign_coeffs(15, 0.2)
+    psi = inputs.gaussian_spinor(d["dims"], 55)
+    diag = inputs.chebyshev_eval(alpha, d["lam"] / 6.5)
+    diag[idx] = np.sign(lam_d)
+    want = (d["W"] * diag) @ (d["W"].conj().T @ psi.ravel())
+    with api.Overlap(d["dims"], dev(torch, d["U"])) as op:
+        op.set_chebyshev(alpha)
+        p = dev(torch, psi)
+        plain = host(op.sign(p)).ravel()
+        op.set_deflation(dev(torch, phi), lam_d)
+        got = host(op.sign(p)).ravel()
+    assert rel_err(got, want) < 1e-11
+    assert rel_err(got, orc.sign(d["dims"], d["U"], alpha, psi, phi, lam_d).ravel()) < TOL_OVL
+    exact = d["S"] @ psi.ravel()
+    assert np.linalg.norm(got - exact) < np.linalg.norm(plain - exact)
