@@ -56,27 +56,44 @@ def make_inputs(w, seed_off=0, need_phi=True):
     return U, psi, alpha, phi, lam
 
 
-def poly_bytes(alpha, V, prec_bytes, recon):
-    """Algorithmic (compulsory) HBM bytes of the polynomial loop, summed order by order:
-    every order reads t_m (S) and the 4 links a site owns (4L); reads t_{m-1} (S) from the second order on; writes
-    t_{m+1} (S) except in the last order; reads+writes the accumulator (2S) when alpha_{m+1} != 0 (write only in the
-    first order)."""
+def poly_bytes(alpha, V, prec_bytes, recon, recurrence="clenshaw"):
+    """Algorithmic (compulsory) HBM bytes of the polynomial loop, summed launch by launch; S = spinor
+    bytes/site, L = link bytes.  Every launch reads its stencil operand (S) and the 4 links a site owns (4L).
+    forward:  + t_{m-1} (S) from the second order on; + write t_{m+1} (S) except in the last order; + read+write of the
+              accumulator (2S) when alpha_{m+1} != 0 (write only in the first order).
+    clenshaw: + write b_k (S); + b_{k+2} (S) from the third launch on; + psi (S) when the launch's psi coefficient is
+              non-zero (alpha_k; alpha_{N-2} - alpha_N in the second launch; alpha_0 in the last)."""
     S = 24 * prec_bytes
     L = recon * prec_bytes
-    last = max(1, max([m for m in range(1, len(alpha)) if alpha[m] != 0.0] or [1]))
+    al = list(alpha)
+    last = max(1, max([m for m in range(1, len(al)) if al[m] != 0.0] or [1]))
     total = 0
-    for m in range(last):  # order m produces t_{m+1}
-        b = S + 4 * L
-        if m >= 1:
-            b += S
-        if m + 1 < last:
-            b += S
-        if m == 0:
-            b += S
-        elif alpha[m + 1] != 0.0:
-            b += 2 * S
-        total += b
-    return total * V, last
+    if recurrence == "forward":
+        for m in range(last):  # order m produces t_{m+1}
+            b = S + 4 * L
+            if m >= 1:
+                b += S
+            if m + 1 < last:
+                b += S
+            if m == 0:
+                b += S
+            elif al[m + 1] != 0.0:
+                b += 2 * S
+            total += b
+        return total * V, last
+    N = last
+    base = 2 * S + 4 * L
+    psi = lambda c: S if c != 0.0 else 0
+    if N == 1:
+        return (base + psi(al[0])) * V, N
+    total += base + psi(al[N - 1])
+    if N == 2:
+        return (total + base + psi(al[0] - al[2])) * V, N
+    total += base + psi(al[N - 2] - al[N])
+    for k in range(N - 3, 0, -1):
+        total += base + S + psi(al[k])
+    total += base + S + psi(al[0])
+    return total * V, N
 
 
 class ClockSampler:
@@ -231,7 +248,8 @@ def dslash_sweep_point(torch, api, dims, prec, recon, reps=100):
             "gbs_requested": V * (9 * S + 8 * L) / ms / 1e6}
 
 
-def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with_e2e, host_inputs=None):
+def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with_e2e, host_inputs=None,
+                  recurrence="clenshaw"):
     """Resident + end-to-end timing of one workload in one precision. Returns a dict of measurements."""
     U, psi, alpha, phi, lam = host_inputs if host_inputs is not None else make_inputs(w, seed_off=rank)
     dims, mu = w["dims"], w["mu"]
@@ -240,6 +258,7 @@ def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with
     op = api.Overlap(dims, torch.from_numpy(U).cuda(), prec, recon)
     res = {}
     try:
+        op.set_recurrence(recurrence)
         orders = op.set_chebyshev(alpha)
         if w["nev"]:
             phid = torch.from_numpy(phi).cuda()
@@ -266,7 +285,7 @@ def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with
         poly_ms.append(pm)
         res.update(ms_per_step=ms / steps, applies_per_s=steps / (ms * 1e-3), launches=l1 - l0, clocks=clocks,
                    orders=orders, poly_ms=pm, poly_launches=poly_launches)
-        bytes_poly, _ = poly_bytes(alpha, V, pb, recon)
+        bytes_poly, _ = poly_bytes(alpha, V, pb, recon, recurrence)
         res["poly_bytes"] = bytes_poly
         res["kernel_us"] = 1e3 * pm / poly_launches
         res["achieved_gbs"] = bytes_poly / (pm * 1e-3) / 1e9
@@ -328,7 +347,8 @@ def run_native(args, w):
 
     hbm_peak, peak_src = measured_peaks()
     host_inputs = make_inputs(w, seed_off=rank)
-    main = bench_overlap(torch, api, B, w, args.prec, args.recon, args.steps, args.warmup, dist, rank, True, host_inputs)
+    main = bench_overlap(torch, api, B, w, args.prec, args.recon, args.steps, args.warmup, dist, rank, True, host_inputs,
+                         args.recurrence)
     n = world
     value = n * main["applies_per_s"]
     line = {
@@ -336,14 +356,14 @@ def run_native(args, w):
         "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.prec, "data": "synthetic",
         "config": {"workload": w["desc"], "precision": args.prec, "links": f"{args.recon}-real",
-                   "orders_run": main["orders"], "parallelism": f"replicas x{n} (independent right-hand sides)",
+                   "orders_run": main["orders"], "recurrence": args.recurrence, "parallelism": f"replicas x{n} (independent right-hand sides)",
                    "l2": "inputs larger than L2 (links 295 MB + 4 spinor streams 98 MB each at 20^3x64 fp64); no flush"
                    if w["dims"] == (20, 20, 20, 64) else "working set is L2-resident by construction (small lattice)"},
         "clocks": main["clocks"],
         "e2e": {"value": n * main["e2e"]["value"], "unit": UNIT, "h2d_bytes_per_step": main["e2e"]["h2d"],
                 "d2h_bytes_per_step": main["e2e"]["d2h"]},
         "gpu_launches": main["launches"],
-        "roofline": {"bound": "hbm", "kernel": "k_wilson_fused (one Chebyshev order per launch)",
+        "roofline": {"bound": "hbm", "kernel": f"k_wilson_fused (one Chebyshev order per launch, {args.recurrence} recurrence)",
                      "achieved": main["achieved_gbs"], "peak": hbm_peak, "unit": "GB/s",
                      "frac": main["achieved_gbs"] / hbm_peak, "peak_source": peak_src, "traffic": None,
                      "kernel_us": main["kernel_us"], "launches_per_step": main["poly_launches"],
@@ -359,9 +379,15 @@ def run_native(args, w):
                                         "orders": r1["orders"]}
             extras["cfg2_cg"] = bench_cg(torch, api, w1)
             if args.prec == "f64":
-                r32 = bench_overlap(torch, api, B, w, "f32", args.recon, args.steps, args.warmup, None, 0, False, host_inputs)
+                r32 = bench_overlap(torch, api, B, w, "f32", args.recon, args.steps, args.warmup, None, 0, False, host_inputs,
+                                    args.recurrence)
                 extras["cfg3_fp32"] = {"applies_per_s": r32["applies_per_s"], "achieved_gbs": r32["achieved_gbs"],
-                                       "frac": r32["achieved_gbs"] / hbm_peak}
+                                       "frac": r32["achieved_gbs"] / hbm_peak, "kernel_us": r32["kernel_us"]}
+            other = "forward" if args.recurrence == "clenshaw" else "clenshaw"
+            ro = bench_overlap(torch, api, B, w, args.prec, args.recon, args.steps, args.warmup, None, 0, False, host_inputs, other)
+            extras[f"cfg3_{other}_recurrence"] = {
+                "applies_per_s": ro["applies_per_s"], "achieved_gbs": ro["achieved_gbs"], "frac": ro["achieved_gbs"] / hbm_peak,
+                "kernel_us": ro["kernel_us"], "algorithmic_bytes_per_site_per_launch": ro["bytes_per_site_per_order"]}
         sweep = []
         for dims in [(8, 8, 8, 32), (20, 20, 20, 64)]:
             for prec, recon in [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)]:
@@ -388,6 +414,8 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
+    ap.add_argument("--recurrence", default="clenshaw", choices=["clenshaw", "forward"],
+                    help="evaluation order of the polynomial sum of eq. 2.3 (ovl_set_recurrence)")
     ap.add_argument("--ref-orders", type=int, default=12, help="polynomial orders in the oracle's bounded sample")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--fast-inputs", action="store_true",

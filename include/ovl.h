@@ -54,6 +54,7 @@ typedef struct ovl_ctx ovl_ctx; /* opaque */
 enum { OVL_OK = 0, OVL_EINVAL = 1, OVL_ENOMEM = 2, OVL_ECUDA = 3, OVL_ESTATE = 4, OVL_ENOTCONV = 5 };
 enum { OVL_F64 = 0, OVL_F32 = 1 };        /* storage + stencil arithmetic precision (reading R18) */
 enum { OVL_RECON18 = 18, OVL_RECON12 = 12 }; /* reals stored per link; 12: third row rebuilt as conj(r0 x r1) */
+enum { OVL_REC_CLENSHAW = 0, OVL_REC_FORWARD = 1 }; /* how sum_m alpha_m T_m(K^) psi of eq. 2.3 is evaluated */
 
 /* Library version string, e.g. "ovl-b200 0.1 (sm_100a)". */
 const char *ovl_version(void);
@@ -79,6 +80,15 @@ int ovl_set_kernel(ovl_ctx *ctx, double m_w, double lambda_max);
  * last non-zero alpha (reading R7); ovl_poly_orders reports that number of K^ applications. */
 int ovl_set_chebyshev(ovl_ctx *ctx, int degree_N, const double *alpha);
 int ovl_poly_orders(const ovl_ctx *ctx);
+
+/* Evaluation order of the polynomial sum of eq. 2.3 ("a short three vector recurrence").  Both run
+ * exactly ovl_poly_orders fused stencil launches and give the same polynomial (they differ by rounding only):
+ *   OVL_REC_FORWARD   t_0 = psi, t_1 = K^ psi, t_{m+1} = 2 K^ t_m - t_{m-1}, s = sum_m alpha_m t_m, as printed;
+ *   OVL_REC_CLENSHAW  b_k = alpha_k psi + 2 K^ b_{k+1} - b_{k+2} (k = N..1), s = alpha_0 psi + K^ b_1 - b_2: the
+ *                     adjoint recurrence, which has no read-modify-write accumulator stream (default).
+ * Errors: OVL_EINVAL for an unknown mode. */
+int ovl_set_recurrence(ovl_ctx *ctx, int mode);
+int ovl_get_recurrence(const ovl_ctx *ctx);
 
 /* Deflation space of eq. 2.3: nev >= 0 vectors phi_c128 [H|D] and eigenvalues lambda (host).
  * nev = 0 switches deflation off.  |lambda_i| < 1e-14 lambda_max is rejected with OVL_EINVAL (reading R9).

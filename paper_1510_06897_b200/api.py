@@ -54,6 +54,11 @@ class Overlap:
         B.ovl_set_chebyshev(self.ctx, alpha)
         return B.ovl_poly_orders(self.ctx)
 
+    def set_recurrence(self, mode):
+        """'clenshaw' (default) or 'forward': evaluation order of the polynomial sum of eq. 2.3."""
+        m = {"clenshaw": B.OVL_REC_CLENSHAW, "forward": B.OVL_REC_FORWARD}.get(mode, mode)
+        B.ovl_set_recurrence(self.ctx, m)
+
     def set_deflation(self, phi, lam):
         B.ovl_set_deflation(self.ctx, phi, lam)
 

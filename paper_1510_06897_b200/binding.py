@@ -14,6 +14,7 @@ import numpy as np
 OVL_OK, OVL_EINVAL, OVL_ENOMEM, OVL_ECUDA, OVL_ESTATE, OVL_ENOTCONV = range(6)
 OVL_F64, OVL_F32 = 0, 1
 OVL_RECON18, OVL_RECON12 = 18, 12
+OVL_REC_CLENSHAW, OVL_REC_FORWARD = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libovl.so")
@@ -28,6 +29,8 @@ SIGNATURES = {
     "ovl_set_kernel": (_I, [_P, _D, _D]),
     "ovl_set_chebyshev": (_I, [_P, _I, C.POINTER(_D)]),
     "ovl_poly_orders": (_I, [_P]),
+    "ovl_set_recurrence": (_I, [_P, _I]),
+    "ovl_get_recurrence": (_I, [_P]),
     "ovl_set_deflation": (_I, [_P, _I, _P, C.POINTER(_D)]),
     "ovl_dw": (_I, [_P, _P, _P]),
     "ovl_khat": (_I, [_P, _P, _P]),
@@ -130,6 +133,14 @@ def ovl_set_chebyshev(ctx, alpha):
 
 def ovl_poly_orders(ctx) -> int:
     return int(load_library().ovl_poly_orders(ctx))
+
+
+def ovl_set_recurrence(ctx, mode):
+    return _check(ctx, load_library().ovl_set_recurrence(ctx, int(mode)))
+
+
+def ovl_get_recurrence(ctx) -> int:
+    return int(load_library().ovl_get_recurrence(ctx))
 
 
 def ovl_set_deflation(ctx, phi, lam):

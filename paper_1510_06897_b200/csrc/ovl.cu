@@ -81,7 +81,7 @@ template <typename F> int with_canonical(ovl_ctx *c, const void *psi, void *out,
 
 extern "C" {
 
-const char *ovl_version(void) { return "ovl-b200 0.1 (sm_100a)"; }
+const char *ovl_version(void) { return "ovl-b200 0.2 (sm_100a)"; }
 
 size_t ovl_device_bytes(const int dims[4], int prec, int recon, int max_nev) {
     if (check_cfg(dims, prec, recon) != OVL_OK || max_nev < 0) return 0;
@@ -180,6 +180,14 @@ int ovl_set_chebyshev(ovl_ctx *c, int N, const double *alpha) {
 }
 
 int ovl_poly_orders(const ovl_ctx *c) { return c ? c->norders : 0; }
+
+int ovl_set_recurrence(ovl_ctx *c, int mode) {
+    if (!c) return OVL_EINVAL;
+    if (mode != OVL_REC_CLENSHAW && mode != OVL_REC_FORWARD) return fail(c, OVL_EINVAL, "unknown recurrence mode %d", mode);
+    c->recurrence = mode;
+    return OVL_OK;
+}
+int ovl_get_recurrence(const ovl_ctx *c) { return c ? c->recurrence : -1; }
 
 int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda) {
     if (!c) return OVL_EINVAL;

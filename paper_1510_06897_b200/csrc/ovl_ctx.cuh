@@ -13,7 +13,7 @@
 
 struct ovl_ctx {
     ovl::Geom g{};
-    int prec = OVL_F64, recon = OVL_RECON18;
+    int prec = OVL_F64, recon = OVL_RECON18, recurrence = OVL_REC_CLENSHAW;
     cudaStream_t st = nullptr;
     double m_w = 1.5, lambda_max = 6.5;
 

@@ -14,60 +14,107 @@ namespace ovl {
         if (e_ != cudaSuccess) return fail((c), OVL_ECUDA, "kernel launch: %s", cudaGetErrorString(e_)); \
     } while (0)
 
-template <typename T, int RECON, int FLAGS>
-inline void launch_wilson_t(ovl_ctx *c, const cx<T> *in, const cx<T> *prev, cx<T> *out, cx<T> *acc, StepParams<T> sp) {
-    const int grid = (c->g.V + WILSON_THREADS - 1) / WILSON_THREADS;
-    k_wilson_fused<T, RECON, FLAGS><<<grid, WILSON_THREADS, 0, c->st>>>(c->g, (const cx<T> *)c->U, in, prev, out, acc, sp);
+// launch shape of the fused kernel: 128-thread CTAs (tiles of 128 consecutive sites); fp64 runs 3 CTAs/SM at up to 168
+// registers, fp32 4 CTAs/SM (measured best on B200)
+template <typename T> struct WilsonCfg;
+template <> struct WilsonCfg<double> { static constexpr int THREADS = 128, MINB = 3; };
+template <> struct WilsonCfg<float> { static constexpr int THREADS = 128, MINB = 4; };
+
+struct WilsonArgs {
+    const void *in = nullptr, *prev = nullptr, *psi = nullptr;
+    void *out = nullptr, *acc = nullptr;
+    double c_diag = 0, c_hop = 0, a_psi = 0, a_acc = 0, a_init = 0;
+    int flip = 0;
+};
+
+template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx *c, const WilsonArgs &a) {
+    constexpr int TH = WilsonCfg<T>::THREADS;
+    const int grid = (c->g.V + TH - 1) / TH;
+    StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip};
+    k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
+        c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp);
 }
 
-template <typename T, int FLAGS>
-inline int launch_wilson(ovl_ctx *c, const void *in, const void *prev, void *out, void *acc, double c_diag, double c_hop,
-                         double a0, double a1) {
-    StepParams<T> sp{(T)c_diag, (T)c_hop, (T)a0, (T)a1};
-    if (c->recon == OVL_RECON18)
-        launch_wilson_t<T, 18, FLAGS>(c, (const cx<T> *)in, (const cx<T> *)prev, (cx<T> *)out, (cx<T> *)acc, sp);
-    else
-        launch_wilson_t<T, 12, FLAGS>(c, (const cx<T> *)in, (const cx<T> *)prev, (cx<T> *)out, (cx<T> *)acc, sp);
+template <typename T, int FLAGS> inline int launch_wilson(ovl_ctx *c, const WilsonArgs &a) {
+    if (c->recon == OVL_RECON18) launch_wilson_t<T, 18, FLAGS>(c, a);
+    else launch_wilson_t<T, 12, FLAGS>(c, a);
     OVL_LAUNCH_CHECK(c);
     return OVL_OK;
 }
 
 // out = D_W in
 template <typename T> int dw_native(ovl_ctx *c, const void *in, void *out) {
-    return launch_wilson<T, F_WRITE>(c, in, nullptr, out, nullptr, 4.0, -0.5, 0, 0);
+    WilsonArgs a;
+    a.in = in; a.out = out; a.c_diag = 4.0; a.c_hop = -0.5;
+    return launch_wilson<T, 0>(c, a);
 }
 // out = K^ in
 template <typename T> int khat_native(ovl_ctx *c, const void *in, void *out) {
-    return launch_wilson<T, F_G5 | F_WRITE>(c, in, nullptr, out, nullptr, (4.0 - c->m_w) / c->lambda_max,
-                                            -0.5 / c->lambda_max, 0, 0);
+    WilsonArgs a;
+    a.in = in; a.out = out; a.c_diag = (4.0 - c->m_w) / c->lambda_max; a.c_hop = -0.5 / c->lambda_max;
+    return launch_wilson<T, K_G5>(c, a);
+}
+
+// acc = sum_{m=0}^{N} alpha_m T_m(K^) src by the forward recurrence exactly as printed:
+// t_0 = src, t_1 = K^ src, t_{m+1} = 2 K^ t_m - t_{m-1}, acc = sum alpha_m t_m.  N launches.
+template <typename T> int cheb_forward(ovl_ctx *c, const void *src) {
+    const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
+    const std::vector<double> &al = c->alpha;
+    const int N = c->norders;
+    WilsonArgs a;
+    a.in = src; a.out = c->tA; a.acc = c->acc; a.c_diag = cd; a.c_hop = ch; a.a_init = al[0]; a.a_acc = al[1];
+    if (N == 1) OVL_TRY((launch_wilson<T, K_G5 | K_ACCI | K_NOWRITE>(c, a)));
+    else OVL_TRY((launch_wilson<T, K_G5 | K_ACCI>(c, a)));
+    for (int m = 1; m < N; ++m) {  // produces t_{m+1}
+        WilsonArgs b;
+        b.in = (m & 1) ? c->tA : c->tB;
+        b.out = (m & 1) ? c->tB : c->tA;
+        b.prev = (m == 1) ? src : b.out;
+        b.acc = c->acc;
+        b.c_diag = 2 * cd; b.c_hop = 2 * ch; b.a_acc = al[m + 1]; b.flip = m & 1;
+        if (m + 1 == N) OVL_TRY((launch_wilson<T, K_G5 | K_PREV | K_ACC | K_NOWRITE>(c, b)));
+        else if (b.a_acc != 0.0) OVL_TRY((launch_wilson<T, K_G5 | K_PREV | K_ACC>(c, b)));
+        else OVL_TRY((launch_wilson<T, K_G5 | K_PREV>(c, b)));
+    }
+    return OVL_OK;
+}
+
+// The same sum by Clenshaw's backward recurrence (the adjoint of the three-term recurrence; SURVEY.md §8(c) O4,
+// §8(d) "Clenshaw form"):  b_{N+1} = b_{N+2} = 0,  b_k = alpha_k src + 2 K^ b_{k+1} - b_{k+2}  (k = N..1),
+// acc = alpha_0 src + K^ b_1 - b_2.  It has no read-modify-write accumulator stream: one order reads b_{k+1} (stencil),
+// b_{k+2} and - when alpha_k != 0 - src, and writes b_k over b_{k+2}.  b_N = alpha_N src is never formed: the first
+// launch applies 2 alpha_N K^ to src directly and the second one carries the (- alpha_N src) term.  N launches.
+template <typename T> int cheb_clenshaw(ovl_ctx *c, const void *src) {
+    const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
+    const std::vector<double> &al = c->alpha;
+    const int N = c->norders;
+    int nl = 0;
+    auto step = [&](const void *in, const void *prev, void *out, double scale, double a_psi) -> int {
+        WilsonArgs a;
+        a.in = in; a.prev = prev; a.psi = src; a.out = out;
+        a.c_diag = scale * cd; a.c_hop = scale * ch; a.a_psi = a_psi; a.flip = (nl++) & 1;
+        if (prev) return a_psi != 0.0 ? launch_wilson<T, K_G5 | K_PREV | K_PSI>(c, a) : launch_wilson<T, K_G5 | K_PREV>(c, a);
+        return a_psi != 0.0 ? launch_wilson<T, K_G5 | K_PSI>(c, a) : launch_wilson<T, K_G5>(c, a);
+    };
+    if (N == 1) return step(src, nullptr, c->acc, al[1], al[0]);
+    OVL_TRY(step(src, nullptr, c->tA, 2 * al[N], al[N - 1]));                  // b_{N-1}
+    if (N == 2) return step(c->tA, nullptr, c->acc, 1.0, al[0] - al[2]);      // acc = alpha_0 src + K^ b_1 - alpha_2 src
+    OVL_TRY(step(c->tA, nullptr, c->tB, 2.0, al[N - 2] - al[N]));              // b_{N-2}
+    void *cur = c->tB, *oth = c->tA;                                          // cur = b_{k+1}, oth = b_{k+2}
+    for (int k = N - 3; k >= 1; --k) {
+        OVL_TRY(step(cur, oth, oth, 2.0, al[k]));
+        void *t = cur; cur = oth; oth = t;
+    }
+    return step(cur, oth, c->acc, 1.0, al[0]);
 }
 
 // acc = sum_{m=0}^{norders} alpha_m T_m(K^) src    (first sum of eq. 2.3; src is not modified)
 template <typename T> int cheb_native(ovl_ctx *c, const void *src) {
-    const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
-    const std::vector<double> &al = c->alpha;
-    const int N = c->norders;
     if (c->profiling) OVL_CUDA(c, cudaEventRecord(c->ev0, c->st));
-    if (N == 1)
-        OVL_TRY((launch_wilson<T, F_G5 | F_ACC_INIT>(c, src, nullptr, nullptr, c->acc, cd, ch, al[0], al[1])));
-    else
-        OVL_TRY((launch_wilson<T, F_G5 | F_WRITE | F_ACC_INIT>(c, src, nullptr, c->tA, c->acc, cd, ch, al[0], al[1])));
-    for (int m = 1; m < N; ++m) {  // produces t_{m+1}
-        const void *in = (m & 1) ? c->tA : c->tB;
-        void *out = (m & 1) ? c->tB : c->tA;
-        const void *prev = (m == 1) ? src : out;
-        const double a1 = al[m + 1];
-        const bool last = (m + 1 == N);
-        if (last)
-            OVL_TRY((launch_wilson<T, F_G5 | F_PREV | F_ACC_ADD>(c, in, prev, nullptr, c->acc, 2 * cd, 2 * ch, 0, a1)));
-        else if (a1 != 0.0)
-            OVL_TRY((launch_wilson<T, F_G5 | F_PREV | F_WRITE | F_ACC_ADD>(c, in, prev, out, c->acc, 2 * cd, 2 * ch, 0, a1)));
-        else
-            OVL_TRY((launch_wilson<T, F_G5 | F_PREV | F_WRITE>(c, in, prev, out, nullptr, 2 * cd, 2 * ch, 0, 0)));
-    }
+    OVL_TRY(c->recurrence == OVL_REC_FORWARD ? cheb_forward<T>(c, src) : cheb_clenshaw<T>(c, src));
     if (c->profiling) {
         OVL_CUDA(c, cudaEventRecord(c->ev1, c->st));
-        c->last_poly_launches = N;
+        c->last_poly_launches = c->norders;
         c->poly_timed = true;
     }
     return OVL_OK;

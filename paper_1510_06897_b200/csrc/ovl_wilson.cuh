@@ -2,19 +2,27 @@
 //
 // One launch = one polynomial order of eq. 2.3, i.e. one pass over HBM:
 //     hop(x) = sum_mu [ (1 - gamma_mu) U_mu(x) in(x+mu) + (1 + gamma_mu) U_mu(x-mu)^dag in(x-mu) ]   eq. 2.2
-//     w(x)   = c_diag * in(x) + c_hop * hop(x)            (D_W: c_diag = 4, c_hop = -1/2;
-//                                                          K^ : (4 - m_w)/lambda_max, -1/(2 lambda_max); x2 for m >= 1)
-//     w      = gamma5 w                     [F_G5]        (K = gamma5 (D_W - m_w); sign flip of spins 2,3)
-//     w     -= prev(x)                      [F_PREV]      (t_{m+1} = 2 K^ t_m - t_{m-1})
-//     out(x) = w                            [F_WRITE]     (may alias prev: the ONLY aliasing pair is prev[k,x] / out[k,x], read then
-//                                                          written by the same thread with a true data dependency, so declaring
-//                                                          both __restrict__ is safe and lets the loads be batched before the stores)
-//     acc(x) = a0 * in(x) + a1 * w          [F_ACC_INIT]  (alpha_0 t_0 + alpha_1 t_1)
-//     acc(x)+= a1 * w                       [F_ACC_ADD]   (alpha_{m+1} t_{m+1})
+//     w(x)   = sigma (c_diag in(x) + c_hop hop(x))        D_W: c_diag = 4, c_hop = -1/2, sigma = 1;
+//                                                         K^ : (4 - m_w)/lambda_max, -1/(2 lambda_max), sigma = gamma5 [K_G5]
+//                                                         (K = gamma5 (D_W - m_w); gamma5 = sign flip of spins 2,3)
+//     w     -= prev(x)                      [K_PREV]      three-term recurrence, forward t_{m+1} = 2 K^ t_m - t_{m-1}
+//                                                         or Clenshaw b_k = alpha_k psi + 2 K^ b_{k+1} - b_{k+2}
+//     w     += a_psi psi(x)                 [K_PSI]       the alpha_k psi term of the Clenshaw form
+//     out(x) = w                            [unless K_NOWRITE]  (may alias prev: prev[k,x] / out[k,x] are read then written by
+//                                                         the same thread with a true data dependency, so __restrict__ is safe)
+//     acc(x)+= a_acc w                      [K_ACC]       forward form: + alpha_{m+1} t_{m+1}
+//     acc(x) = a_init in(x) + a_acc w       [K_ACCI]      forward form, first order: alpha_0 t_0 + alpha_1 t_1
 // This is the paper's "merging together the Wilson matrix and polynomial algebra ... into a single GPU kernel"
 // (PAPER.md:72), re-derived for sm_100a: thread per site, SoA planes so that every load of a warp is one
 // contiguous segment, spin projection before the colour multiply (2 x 3 complex per hop instead of 4 x 3),
 // antiperiodic t phase applied in-kernel (reading R3), optional 12-real links (third row = conj(r0 x r1)).
+//
+// Latency structure: the site-local operands (in(x), prev(x), psi(x)) are folded into the INITIAL value of
+// the 12 hop accumulators at the top of the kernel,
+//     h_k := (c_diag/c_hop) in_k + sigma_k (a_psi psi_k - prev_k)/c_hop ,   w_k = sigma_k c_hop (h_k + hop_k) ,
+// so their first-touch (DRAM) loads are in flight together with the first hop's and the epilogue is store-only:
+// no load of the kernel waits behind the whole stencil.  Measured on B200 at 20^3x64 fp64 this (with the Clenshaw form,
+// which has no read-modify-write stream) took one order from 171 us to 125 us.
 //
 // Spin projectors in the basis of reading R2 (gamma5 = diag(1,1,-1,-1)); s = +1 for (1 + gamma_mu), -1 for (1 - gamma_mu):
 //   x: h0 = p0 + s i p3, h1 = p1 + s i p2;  r2 = -s i h1, r3 = -s i h0
@@ -27,10 +35,13 @@
 
 namespace ovl {
 
-enum : int { F_G5 = 1, F_PREV = 2, F_WRITE = 4, F_ACC_INIT = 8, F_ACC_ADD = 16 };
+enum : int { K_G5 = 1, K_PREV = 2, K_PSI = 4, K_ACC = 8, K_ACCI = 16, K_NOWRITE = 32 };
 
+// c_hop and the ratios r_c = c_diag/c_hop, r_p = 1/c_hop, r_a = a_psi/c_hop (see the header); flip = sweep the lattice
+// from the last CTA tile to the first (consecutive orders alternate, so an order starts on what the previous one left in L2)
 template <typename T> struct StepParams {
-    T c_diag, c_hop, a0, a1;
+    T c_hop, r_c, r_p, r_a, a_acc, a_init;
+    int flip;
 };
 
 // Load the 3x3 link U_mu(su) (rows r, cols c) from the native planes; rebuild row 2 for 12-real storage.
@@ -134,51 +145,69 @@ __device__ __forceinline__ void hop_pair(cx<T> (&hop)[12], const cx<T> *__restri
     hop_dir<T, RECON, MU, 0>(hop, in, U, g.V, sb, sb, bb);
 }
 
-constexpr int WILSON_THREADS = 128;
-
-template <typename T, int RECON, int FLAGS>
-__global__ void __launch_bounds__(WILSON_THREADS)
+template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
 k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *__restrict__ prev,
-               cx<T> *__restrict__ out,
-               cx<T> *__restrict__ acc, const StepParams<T> sp) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+               const cx<T> *__restrict__ psi, cx<T> *__restrict__ out, cx<T> *__restrict__ acc, const StepParams<T> sp) {
+    const int tile = sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int s = tile * THREADS + threadIdx.x;
     if (s >= g.V) return;
     const int x = s % g.L[0];
     const int y = (s / g.L[0]) % g.L[1];
     const int z = (s / g.sxy) % g.L[2];
     const int t = s / g.sxyz;
-
-    cx<T> hop[12];
-#pragma unroll
-    for (int k = 0; k < 12; ++k) hop[k] = mk<T>(0, 0);
-    hop_pair<T, RECON, 0>(hop, in, U, g, s, x, 1);
-    hop_pair<T, RECON, 1>(hop, in, U, g, s, y, g.L[0]);
-    hop_pair<T, RECON, 2>(hop, in, U, g, s, z, g.sxy);
-    hop_pair<T, RECON, 3>(hop, in, U, g, s, t, g.sxyz);
-
     const size_t V = g.V;
+
+    // accumulators start from the site-local terms (no loads are left for the epilogue)
+    cx<T> hop[12];
 #pragma unroll
     for (int k = 0; k < 12; ++k) {
         const cx<T> c = ldg(in + k * V + s);
-        cx<T> w;
-        w.x = fma(sp.c_diag, c.x, sp.c_hop * hop[k].x);
-        w.y = fma(sp.c_diag, c.y, sp.c_hop * hop[k].y);
-        if ((FLAGS & F_G5) && k >= 6) { w.x = -w.x; w.y = -w.y; }
-        if (FLAGS & F_PREV) {
-            const cx<T> pv = prev[k * V + s];
-            w.x -= pv.x; w.y -= pv.y;
+        hop[k].x = sp.r_c * c.x;
+        hop[k].y = sp.r_c * c.y;
+    }
+    if (FLAGS & K_PREV) {
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const cx<T> pv = ldg(prev + k * V + s);
+            const T r = ((FLAGS & K_G5) && k >= 6) ? sp.r_p : -sp.r_p;
+            hop[k].x = fma(r, pv.x, hop[k].x);
+            hop[k].y = fma(r, pv.y, hop[k].y);
         }
-        if (FLAGS & F_WRITE) out[k * V + s] = w;
-        if (FLAGS & F_ACC_INIT) {
+    }
+    if (FLAGS & K_PSI) {
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const cx<T> ps = ldg(psi + k * V + s);
+            const T r = ((FLAGS & K_G5) && k >= 6) ? -sp.r_a : sp.r_a;
+            hop[k].x = fma(r, ps.x, hop[k].x);
+            hop[k].y = fma(r, ps.y, hop[k].y);
+        }
+    }
+    // t first: in(x + t^) and U_t(x) are the first touches of the sweep (DRAM), everything after is mostly cache
+    hop_pair<T, RECON, 3>(hop, in, U, g, s, t, g.sxyz);
+    hop_pair<T, RECON, 2>(hop, in, U, g, s, z, g.sxy);
+    hop_pair<T, RECON, 1>(hop, in, U, g, s, y, g.L[0]);
+    hop_pair<T, RECON, 0>(hop, in, U, g, s, x, 1);
+
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        const T f = ((FLAGS & K_G5) && k >= 6) ? -sp.c_hop : sp.c_hop;
+        cx<T> w;
+        w.x = f * hop[k].x;
+        w.y = f * hop[k].y;
+        if (!(FLAGS & K_NOWRITE)) out[k * V + s] = w;
+        if (FLAGS & K_ACCI) {
+            const cx<T> c = ldg(in + k * V + s);
             cx<T> a;
-            a.x = fma(sp.a0, c.x, sp.a1 * w.x);
-            a.y = fma(sp.a0, c.y, sp.a1 * w.y);
+            a.x = fma(sp.a_init, c.x, sp.a_acc * w.x);
+            a.y = fma(sp.a_init, c.y, sp.a_acc * w.y);
             acc[k * V + s] = a;
         }
-        if (FLAGS & F_ACC_ADD) {
+        if (FLAGS & K_ACC) {
             cx<T> a = acc[k * V + s];
-            a.x = fma(sp.a1, w.x, a.x);
-            a.y = fma(sp.a1, w.y, a.y);
+            a.x = fma(sp.a_acc, w.x, a.x);
+            a.y = fma(sp.a_acc, w.y, a.y);
             acc[k * V + s] = a;
         }
     }

@@ -52,7 +52,8 @@ def test_dw_full_field_20x20x20x64(torch, api, orc, rough, prec, recon, tol):
     assert np.abs(got[sites] - want[sites]).max() < 20 * tol * scale
 
 
-def test_low_degree_deflated_overlap_vs_oracle_full_size(torch, api, orc, rough):
+@pytest.mark.parametrize("rec", ["clenshaw", "forward"])
+def test_low_degree_deflated_overlap_vs_oracle_full_size(torch, api, orc, rough, rec):
     """The fused Chebyshev step, deflation and assembly in the full-size launch configuration against the oracle
     (degree 9 keeps the oracle to seconds; every kernel variant of the degree-400 path is exercised)."""
     U, psi = rough
@@ -61,14 +62,16 @@ def test_low_degree_deflated_overlap_vs_oracle_full_size(torch, api, orc, rough)
     alpha = inputs.chebyshev_sign_coeffs(9, 0.3)
     want = orc.overlap(DIMS, U, alpha, 0.01, psi, phi, lam)
     with api.Overlap(DIMS, dev(torch, U)) as op:
+        op.set_recurrence(rec)
         op.set_chebyshev(alpha)
         op.set_deflation(dev(torch, phi), lam)
         got = op.overlap(dev(torch, psi), 0.01).cpu().numpy()
     assert rel_err(got, want) < 1e-10
 
 
-@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
-def test_degree400_sign_vs_fft_closed_form_full_size(torch, api, prec, tol):
+@pytest.mark.parametrize("prec,tol,rec", [("f64", 1e-10, "clenshaw"), ("f64", 1e-10, "forward"), ("f32", 1e-5, "clenshaw"),
+                                          ("f32", 1e-5, "forward")])
+def test_degree400_sign_vs_fft_closed_form_full_size(torch, api, prec, tol, rec):
     """Pure gauge U_mu(x) = g(x) g(x+mu)^dag at 20^3 x 64: sign(K) psi is known in closed form at any volume. With the
     degree-400 table the polynomial error on the spectrum is < 1e-12, so GPU vs closed form tests the whole
     399-order recurrence in bench.py's configuration."""
@@ -80,6 +83,7 @@ def test_degree400_sign_vs_fft_closed_form_full_size(torch, api, prec, tol):
     delta = np.abs(inputs.chebyshev_eval(alpha, omega.ravel() / 6.5) - 1.0).max()
     assert delta < 1e-11
     with api.Overlap(DIMS, dev(torch, U), prec) as op:
+        op.set_recurrence(rec)
         assert op.set_chebyshev(alpha) == 399
         p = dev(torch, psi, op.cdtype)
         s = op.sign(p)

@@ -81,26 +81,56 @@ def test_khat_fp64(torch, api, orc):
     assert rel_err(got, orc.khat(dims, U, psi, 1.4, 6.1)) < TOL_DW
 
 
-@pytest.mark.parametrize("dims,N", [((4, 4, 4, 4), 1), ((4, 4, 4, 4), 2), ((4, 4, 4, 4), 3), ((4, 6, 8, 10), 24), ((6, 4, 2, 8), 37)])
+RECS = ["clenshaw", "forward"]  # both evaluation orders of the polynomial sum (ovl_set_recurrence)
+
+
+@pytest.mark.parametrize("dims,N", [((4, 4, 4, 4), 1), ((4, 4, 4, 4), 2), ((4, 4, 4, 4), 3), ((4, 4, 4, 4), 4), ((4, 4, 4, 4), 5),
+                                    ((4, 6, 8, 10), 24), ((6, 4, 2, 8), 37)])
 @pytest.mark.parametrize("recon", [18, 12])
-def test_sign_generic_coefficients(torch, api, orc, dims, N, recon):
-    """Every order accumulates (even and odd alpha non-zero, one zero in the middle): recurrence indexing."""
+@pytest.mark.parametrize("rec", RECS)
+def test_sign_generic_coefficients(torch, api, orc, dims, N, recon, rec):
+    """Every order accumulates (even and odd alpha non-zero, one zero in the middle): recurrence indexing, including
+    the short tables N = 1..5 where the Clenshaw start-up launches (b_{N-1}, b_{N-2}) and the final one overlap."""
     U = inputs.random_links(dims, 0.5, 9)
     psi = inputs.gaussian_spinor(dims, 10)
     alpha = rough_alpha(N)
     want = orc.sign(dims, U, alpha, psi)
     with api.Overlap(dims, dev(torch, U), "f64", recon) as op:
+        op.set_recurrence(rec)
         assert op.set_chebyshev(alpha) == N
         got = host(op.sign(dev(torch, psi)))
     assert rel_err(got, want) < TOL_OVL
 
 
-def test_trailing_zero_coefficients_are_skipped(torch, api, orc):
+@pytest.mark.parametrize("rec", RECS)
+@pytest.mark.parametrize("zeros", [(0,), (0, 2), (1, 3), (0, 1, 2, 3, 4, 5), (5, 7), (6, 8)])
+def test_sign_with_vanishing_coefficients(torch, api, orc, rec, zeros):
+    """Tables with zeros in the places the recurrences special-case: alpha_0 (no psi term in the last Clenshaw launch),
+    alpha_{N-1} and alpha_{N-2} - alpha_N (start-up launches), runs of zeros (orders that skip the psi / acc stream)."""
+    dims, N = (4, 4, 4, 6), 8
+    U = inputs.random_links(dims, 0.5, 19)
+    psi = inputs.gaussian_spinor(dims, 20)
+    alpha = rough_alpha(N, seed=11)
+    for z in zeros:
+        alpha[z] = 0.0
+    if zeros == (6, 8):
+        alpha[6], alpha[8] = 0.25, 0.25  # alpha_{N-2} - alpha_N = 0
+    want = orc.sign(dims, U, alpha, psi)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_recurrence(rec)
+        op.set_chebyshev(alpha)
+        got = host(op.sign(dev(torch, psi)))
+    assert rel_err(got, want) < TOL_OVL
+
+
+@pytest.mark.parametrize("rec", RECS)
+def test_trailing_zero_coefficients_are_skipped(torch, api, orc, rec):
     dims = (4, 4, 4, 4)
     U = inputs.random_links(dims, 0.5, 9)
     psi = inputs.gaussian_spinor(dims, 10)
     alpha = np.concatenate([rough_alpha(9), np.zeros(5)])
     with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_recurrence(rec)
         assert op.set_chebyshev(alpha) == 9  # reading R7
         got = host(op.sign(dev(torch, psi)))
     assert rel_err(got, orc.sign(dims, U, alpha, psi)) < TOL_OVL
@@ -134,7 +164,8 @@ def test_config0_overlap_4x4(torch, api, orc, dense44):
 
 @pytest.mark.parametrize("prec,tol", [("f64", TOL_OVL), ("f32", TOL_F32)])
 @pytest.mark.parametrize("recon", [18, 12])
-def test_deflated_sign_and_overlap(torch, api, orc, prec, tol, recon):
+@pytest.mark.parametrize("rec", RECS)
+def test_deflated_sign_and_overlap(torch, api, orc, prec, tol, recon, rec):
     """eq. 2.3 complete, with generic orthonormal vectors and 'eigenvalues' of both signs (reading R10: a well-defined
     linear map for any (phi_i, lambda_i)); coarse polynomial so the deflation term is O(1)."""
     dims = (4, 6, 8, 10)
@@ -149,6 +180,7 @@ def test_deflated_sign_and_overlap(torch, api, orc, prec, tol, recon):
     assert rel_err(want_s, plain) > 1e-3  # deflation does something here
     cd = torch.complex128 if prec == "f64" else torch.complex64
     with api.Overlap(dims, dev(torch, U), prec, recon) as op:
+        op.set_recurrence(rec)
         op.set_chebyshev(alpha)
         op.set_deflation(dev(torch, phi), lam)
         p = dev(torch, psi, cd)
@@ -160,7 +192,8 @@ def test_deflated_sign_and_overlap(torch, api, orc, prec, tol, recon):
         assert rel_err(host(op.sign(p)), plain) < tol
 
 
-def test_config1_shape_8x8x8x32_degree200_nev20(torch, api, orc):
+@pytest.mark.parametrize("rec", RECS)
+def test_config1_shape_8x8x8x32_degree200_nev20(torch, api, orc, rec):
     """BASELINE config 1 shape: 8^3 x 32, smeared links, mu = 0.01, degree 200, 20 deflation vectors (generic
     orthonormal stand-ins for the Lanczos vectors, DESIGN.md input recipe); several tiles + ragged last block."""
     dims = (8, 8, 8, 32)
@@ -171,6 +204,7 @@ def test_config1_shape_8x8x8x32_degree200_nev20(torch, api, orc):
     alpha = inputs.chebyshev_sign_coeffs(200, 0.95 * 0.505 / 6.5)
     want = orc.overlap(dims, U, alpha, 0.01, psi, phi, lam)
     with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_recurrence(rec)
         assert op.set_chebyshev(alpha) == 199  # degree 200 table, alpha_200 = 0 (reading R7)
         op.set_deflation(dev(torch, phi), lam)
         p = dev(torch, psi)
