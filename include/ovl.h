@@ -90,6 +90,11 @@ int ovl_poly_orders(const ovl_ctx *ctx);
 int ovl_set_recurrence(ovl_ctx *ctx, int mode);
 int ovl_get_recurrence(const ovl_ctx *ctx);
 
+/* The polynomial loop is a fixed launch sequence per source field; by default it is captured once into a CUDA graph and
+ * replayed (launch overhead 0.5 us instead of 2 us per order).  Graphs need a real stream: a context created on the
+ * legacy default stream (cuda_stream = 0) always launches directly.  on = 0 forces direct launches. */
+int ovl_set_graphs(ovl_ctx *ctx, int on);
+
 /* Deflation space of eq. 2.3: nev >= 0 vectors phi_c128 [H|D] and eigenvalues lambda (host).
  * nev = 0 switches deflation off.  |lambda_i| < 1e-14 lambda_max is rejected with OVL_EINVAL (reading R9).
  * The vectors are used exactly as given (no re-orthonormalisation; reading R10). */

@@ -59,6 +59,10 @@ class Overlap:
         m = {"clenshaw": B.OVL_REC_CLENSHAW, "forward": B.OVL_REC_FORWARD}.get(mode, mode)
         B.ovl_set_recurrence(self.ctx, m)
 
+    def set_graphs(self, on=True):
+        """CUDA-graph replay of the polynomial loop (only effective when the context runs on a non-default stream)."""
+        B.ovl_set_graphs(self.ctx, on)
+
     def set_deflation(self, phi, lam):
         B.ovl_set_deflation(self.ctx, phi, lam)
 

@@ -31,6 +31,7 @@ SIGNATURES = {
     "ovl_poly_orders": (_I, [_P]),
     "ovl_set_recurrence": (_I, [_P, _I]),
     "ovl_get_recurrence": (_I, [_P]),
+    "ovl_set_graphs": (_I, [_P, _I]),
     "ovl_set_deflation": (_I, [_P, _I, _P, C.POINTER(_D)]),
     "ovl_dw": (_I, [_P, _P, _P]),
     "ovl_khat": (_I, [_P, _P, _P]),
@@ -141,6 +142,10 @@ def ovl_set_recurrence(ctx, mode):
 
 def ovl_get_recurrence(ctx) -> int:
     return int(load_library().ovl_get_recurrence(ctx))
+
+
+def ovl_set_graphs(ctx, on=True):
+    return _check(ctx, load_library().ovl_set_graphs(ctx, int(bool(on))))
 
 
 def ovl_set_deflation(ctx, phi, lam):

@@ -148,6 +148,8 @@ int ovl_destroy(ovl_ctx *c) {
                     c->stage_in, c->stage_out, c->proj_partial, c->w_dev, c->coef_dev, c->red_partial, c->sc_dev};
     for (void *b : bufs)
         if (b) cudaFree(b);
+    for (auto &e : c->graphs)
+        if (e.exec) cudaGraphExecDestroy(e.exec);
     if (c->sc_host) cudaFreeHost(c->sc_host);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -162,6 +164,7 @@ int ovl_set_kernel(ovl_ctx *c, double m_w, double lambda_max) {
     c->m_w = m_w;
     c->lambda_max = lambda_max;
     c->coef_stale = true;
+    ++c->poly_gen;
     return OVL_OK;
 }
 
@@ -176,6 +179,7 @@ int ovl_set_chebyshev(ovl_ctx *c, int N, const double *alpha) {
         if (alpha[m] != 0.0) last = m;
     c->norders = last;
     c->coef_stale = true;
+    ++c->poly_gen;
     return OVL_OK;
 }
 
@@ -185,9 +189,16 @@ int ovl_set_recurrence(ovl_ctx *c, int mode) {
     if (!c) return OVL_EINVAL;
     if (mode != OVL_REC_CLENSHAW && mode != OVL_REC_FORWARD) return fail(c, OVL_EINVAL, "unknown recurrence mode %d", mode);
     c->recurrence = mode;
+    ++c->poly_gen;
     return OVL_OK;
 }
 int ovl_get_recurrence(const ovl_ctx *c) { return c ? c->recurrence : -1; }
+
+int ovl_set_graphs(ovl_ctx *c, int on) {
+    if (!c) return OVL_EINVAL;
+    c->use_graphs = on != 0;
+    return OVL_OK;
+}
 
 int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda) {
     if (!c) return OVL_EINVAL;

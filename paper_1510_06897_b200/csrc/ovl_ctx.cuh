@@ -36,6 +36,17 @@ struct ovl_ctx {
     double *red_partial = nullptr, *sc_dev = nullptr, *sc_host = nullptr;
     int red_nblk = 0;
 
+    // CUDA graphs of the polynomial loop (one per source field), replayed instead of re-issuing norders launches
+    struct PolyGraph {
+        const void *src = nullptr;
+        unsigned long long gen = 0, last_use = 0;
+        cudaGraphExec_t exec = nullptr;
+    };
+    static constexpr int NGRAPH = 8;
+    PolyGraph graphs[NGRAPH];
+    unsigned long long poly_gen = 1, use_clock = 0;  // poly_gen changes whenever the launch sequence would
+    bool use_graphs = true;
+
     // measurement
     bool profiling = false;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;

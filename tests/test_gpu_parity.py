@@ -285,6 +285,46 @@ def test_host_pointers_and_native_fields(torch, api, orc):
         assert rel_err(op.sign(psi), orc.sign(dims, U, alpha, psi, phi, lam)) < TOL_OVL
 
 
+@pytest.mark.parametrize("rec", RECS)
+def test_graph_replay_equals_direct_launches(torch, api, orc, rec):
+    """On a real (non-default) stream the polynomial loop is replayed from a CUDA graph; results must be bit-identical
+    to direct launches, also after the table, the kernel parameters or the source buffer change (graph invalidation)."""
+    dims = (4, 6, 8, 10)
+    U = inputs.random_links(dims, 0.4, 41)
+    psi = inputs.gaussian_spinor(dims, 42)
+    chi = inputs.gaussian_spinor(dims, 43)
+    a1, a2 = rough_alpha(17, seed=3), rough_alpha(12, seed=4)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with api.Overlap(dims, dev(torch, U), stream=side) as op:
+            op.set_recurrence(rec)
+            res = {}
+            for graphs in (True, False):
+                op.set_graphs(graphs)
+                out = []
+                op.set_chebyshev(a1)
+                p, q = dev(torch, psi), dev(torch, chi)
+                out.append(host(op.sign(p)))
+                out.append(host(op.sign(p)))      # replay
+                out.append(host(op.sign(q)))
+                op.set_chebyshev(a2)              # new table -> new launch sequence
+                out.append(host(op.sign(p)))
+                B_ = __import__("paper_1510_06897_b200.binding", fromlist=["x"])
+                B_.ovl_set_kernel(op.ctx, 1.4, 6.2)
+                out.append(host(op.sign(p)))
+                B_.ovl_set_kernel(op.ctx, 1.5, 6.5)
+                nat_in, nat_out = op.to_native(p), op.native_empty()
+                op.overlap_native(nat_in, nat_out, 0.03)
+                out.append(host(op.from_native(nat_out)))
+                res[graphs] = out
+            side.synchronize()
+    for g, d in zip(res[True], res[False]):
+        assert np.array_equal(g, d)
+    assert rel_err(res[True][0], orc.sign(dims, U, a1, psi)) < TOL_OVL
+    assert rel_err(res[True][3], orc.sign(dims, U, a2, psi)) < TOL_OVL
+    assert rel_err(res[True][4], orc.sign(dims, U, a2, psi, m_w=1.4, lambda_max=6.2)) < TOL_OVL
+
+
 def test_bit_identical_run_to_run(torch, api):
     dims = (6, 6, 6, 10)
     U = dev(torch, inputs.random_links(dims, 0.4, 61))
