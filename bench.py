@@ -39,6 +39,11 @@ WORKLOADS = {
     "tiny": dict(dims=(4, 4, 4, 8), link_eps=0.3, stout=1, mu=0.01, degree=40, nev=4, poly_eps=0.09,
                  desc="4^3x8 smoke-sized workload (not a benchmark)"),
 }
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full` capture
+# (profiles/r1b_full.md: 681.0 MB with the psi term, 594.2 MB without, 198 : 199 launches per apply) -- bench.py cannot
+# run ncu itself; the value is reported only for the exact configuration that capture was taken on.
+NCU_TRAFFIC = {("cfg3", "f64", 18, "clenshaw"): {"bytes_per_launch": (198 * 681.1e6 + 199 * 594.2e6) / 397,
+                                                 "source": "profiles/r1b_full.md"}}
 METRIC = "overlap D[mu]psi applies/s"
 UNIT = "applies/s"
 
@@ -364,7 +369,10 @@ def run_native(args, w):
         "gpu_launches": main["launches"],
         "roofline": {"bound": "hbm", "kernel": f"k_wilson_fused (one Chebyshev order per launch, {args.recurrence} recurrence)",
                      "achieved": main["achieved_gbs"], "peak": hbm_peak, "unit": "GB/s",
-                     "frac": main["achieved_gbs"] / hbm_peak, "peak_source": peak_src, "traffic": None,
+                     "frac": main["achieved_gbs"] / hbm_peak, "peak_source": peak_src,
+                     "traffic": (NCU_TRAFFIC.get((args.workload, args.prec, args.recon, args.recurrence)) or {}).get("bytes_per_launch"),
+                     "traffic_source": (NCU_TRAFFIC.get((args.workload, args.prec, args.recon, args.recurrence)) or {}).get("source"),
+                     "algorithmic_bytes_per_launch": main["poly_bytes"] / main["poly_launches"],
                      "kernel_us": main["kernel_us"], "launches_per_step": main["poly_launches"],
                      "algorithmic_bytes_per_site_per_launch": main["bytes_per_site_per_order"],
                      "frac_of_nominal_8TBs": main["achieved_gbs"] / 8000.0},
