@@ -309,6 +309,30 @@ def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with
     return res
 
 
+def bench_multi(torch, api, w, prec, recon, nrhs, steps, warmup, host_inputs=None):
+    """nrhs right-hand sides per call (ovl_overlap_multi_native); applies/s counts every
+    right-hand side.  Inputs resident, native layout."""
+    U, psi, alpha, phi, lam = host_inputs if host_inputs is not None else make_inputs(w)
+    with api.Overlap(w["dims"], torch.from_numpy(U).cuda(), prec, recon) as op:
+        orders = op.set_chebyshev(alpha)
+        if w["nev"]:
+            phid = torch.from_numpy(phi).cuda()
+            op.set_deflation(phid, lam)
+            del phid
+        fb = op.native_empty().numel()
+        nin, nout = op.native_empty(nrhs), op.native_empty(nrhs)
+        p = torch.from_numpy(psi).cuda().to(op.cdtype)
+        for r in range(nrhs):
+            nin[r * fb:(r + 1) * fb].copy_(op.to_native(torch.roll(p, r, 0).contiguous()))
+        op.set_profiling(True)
+        for _ in range(warmup):
+            op.overlap_multi_native(nin, nout, nrhs, w["mu"])
+        ms = time_region(torch, op.stream, lambda: op.overlap_multi_native(nin, nout, nrhs, w["mu"]), steps)
+        pm, launches = op.last_poly_timing()
+    return {"nrhs": nrhs, "applies_per_s": nrhs * steps / (ms * 1e-3), "ms_per_call": ms / steps,
+            "us_per_order_per_rhs": 1e3 * pm / launches / nrhs, "orders": orders}
+
+
 def bench_cg(torch, api, w, steps_tol=1e-8):
     """BASELINE config 2: CG on D^dag D x = b at mu = 0.05 on the cfg1 lattice, deflated sign function in every apply."""
     U, b, alpha, phi, lam = make_inputs(w, seed_off=7)
@@ -385,6 +409,9 @@ def run_native(args, w):
             extras["cfg1_8x8x8x32"] = {"applies_per_s": r1["applies_per_s"], "us_per_order": r1["kernel_us"],
                                         "orders": r1["orders"]}
             extras["cfg2_cg"] = bench_cg(torch, api, w1)
+            extras["multi_rhs"] = {
+                "cfg3_20x20x20x64_fp64_4rhs": bench_multi(torch, api, w, "f64", args.recon, 4, 2, 2, host_inputs),
+                "cfg1_8x8x8x32_fp64_12rhs": bench_multi(torch, api, w1, "f64", 18, 12, 10, 3)}
             if args.prec == "f64":
                 r32 = bench_overlap(torch, api, B, w, "f32", args.recon, args.steps, args.warmup, None, 0, False, host_inputs,
                                     args.recurrence)

@@ -54,6 +54,7 @@ typedef struct ovl_ctx ovl_ctx; /* opaque */
 enum { OVL_OK = 0, OVL_EINVAL = 1, OVL_ENOMEM = 2, OVL_ECUDA = 3, OVL_ESTATE = 4, OVL_ENOTCONV = 5 };
 enum { OVL_F64 = 0, OVL_F32 = 1 };        /* storage + stencil arithmetic precision (reading R18) */
 enum { OVL_RECON18 = 18, OVL_RECON12 = 12 }; /* reals stored per link; 12: third row rebuilt as conj(r0 x r1) */
+#define OVL_MAX_RHS 12                        /* right-hand sides per multi call (12 = one propagator's spin-colour sources) */
 enum { OVL_REC_CLENSHAW = 0, OVL_REC_FORWARD = 1 }; /* how sum_m alpha_m T_m(K^) psi of eq. 2.3 is evaluated */
 
 /* Library version string, e.g. "ovl-b200 0.1 (sm_100a)". */
@@ -113,6 +114,15 @@ int ovl_sign(ovl_ctx *ctx, const void *psi, void *out);
  * (dagger = 1, reading R12). */
 int ovl_overlap(ovl_ctx *ctx, double mu, int dagger, const void *psi, void *out);
 
+/* out_r = D[mu] psi_r (or D[mu]^dag psi_r) for r < nrhs right-hand sides in one call, 1 <= nrhs <= OVL_MAX_RHS
+ * (the paper's end use is propagators, i.e. 12 sources per configuration).
+ * psi, out [H|D]: nrhs consecutive canonical spinors, [nrhs][V][4][3].  Every launch of the fused Wilson/Chebyshev
+ * kernel works on all right-hand sides, so the links (576 of the 1248 B/site/order in fp64) are read from HBM once per
+ * tile instead of once per right-hand side; each out_r is bit-identical to what ovl_overlap returns for psi_r.
+ * The recurrence workspace grows to 4 * nrhs fields on first use.  Errors: OVL_EINVAL (nrhs out of range, null or
+ * aliased pointers), OVL_ESTATE (no polynomial), OVL_ENOMEM. */
+int ovl_overlap_multi(ovl_ctx *ctx, int nrhs, double mu, int dagger, const void *psi, void *out);
+
 /* Conjugate gradient on D[mu]^dag D[mu] x = b, x0 = 0, stop when the recursive residual ||r_k|| <= tol ||b||
  * or after maxiter iterations (tol <= 0: exactly maxiter iterations, status OVL_OK).  b, x [H|D] canonical.
  * *iters_out = iterations done, *true_relres_out = ||b - A x|| / ||b|| recomputed at the end.
@@ -129,6 +139,8 @@ int ovl_field_import(ovl_ctx *ctx, const void *canonical /*[H|D]*/, void *native
 int ovl_field_export(ovl_ctx *ctx, const void *native /*D*/, void *canonical /*[H|D]*/);
 int ovl_dw_native(ovl_ctx *ctx, const void *in_native, void *out_native);
 int ovl_overlap_native(ovl_ctx *ctx, double mu, int dagger, const void *in_native, void *out_native);
+/* nrhs consecutive native fields (nrhs * ovl_field_bytes bytes each side), see ovl_overlap_multi */
+int ovl_overlap_multi_native(ovl_ctx *ctx, int nrhs, double mu, int dagger, const void *in_native, void *out_native);
 
 /* ---- measurement hooks ------------------------------------------------------------------------------------------
  * With profiling on, ovl_sign / ovl_overlap(_native) bracket the polynomial loop (the launches of the fused

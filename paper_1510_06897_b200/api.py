@@ -90,6 +90,12 @@ class Overlap:
     def overlap(self, psi, mu, dagger=False):
         return self._run(B.ovl_overlap, psi, mu, int(dagger))
 
+    def overlap_multi(self, psi, mu, dagger=False):
+        """psi: (nrhs, V, 4, 3); returns D[mu] psi_r for every r with the links read once per tile for all of them."""
+        out = self._like(psi)
+        B.ovl_overlap_multi(self.ctx, int(psi.shape[0]), mu, int(dagger), psi, out)
+        return out
+
     def cg(self, b, mu, tol=1e-8, maxiter=1000):
         """Solve D^dag D x = b. Returns (x, iterations, true relative residual, converged)."""
         x = self._like(b)
@@ -97,9 +103,9 @@ class Overlap:
         return x, it, rel, rc == B.OVL_OK
 
     # ---- native-layout fields
-    def native_empty(self):
+    def native_empty(self, nrhs=1):
         torch = _torch()
-        return torch.empty(B.ovl_field_bytes(self.ctx), dtype=torch.uint8, device="cuda")
+        return torch.empty(B.ovl_field_bytes(self.ctx) * nrhs, dtype=torch.uint8, device="cuda")
 
     def to_native(self, psi):
         nat = self.native_empty()
@@ -117,6 +123,9 @@ class Overlap:
 
     def overlap_native(self, nat_in, nat_out, mu, dagger=False):
         B.ovl_overlap_native(self.ctx, mu, int(dagger), nat_in, nat_out)
+
+    def overlap_multi_native(self, nat_in, nat_out, nrhs, mu, dagger=False):
+        B.ovl_overlap_multi_native(self.ctx, nrhs, mu, int(dagger), nat_in, nat_out)
 
     # ---- measurement
     def set_profiling(self, on=True):

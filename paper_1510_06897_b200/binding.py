@@ -15,6 +15,7 @@ OVL_OK, OVL_EINVAL, OVL_ENOMEM, OVL_ECUDA, OVL_ESTATE, OVL_ENOTCONV = range(6)
 OVL_F64, OVL_F32 = 0, 1
 OVL_RECON18, OVL_RECON12 = 18, 12
 OVL_REC_CLENSHAW, OVL_REC_FORWARD = 0, 1
+OVL_MAX_RHS = 12
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libovl.so")
@@ -37,6 +38,7 @@ SIGNATURES = {
     "ovl_khat": (_I, [_P, _P, _P]),
     "ovl_sign": (_I, [_P, _P, _P]),
     "ovl_overlap": (_I, [_P, _D, _I, _P, _P]),
+    "ovl_overlap_multi": (_I, [_P, _I, _D, _I, _P, _P]),
     "ovl_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_last_error": (C.c_char_p, [_P]),
     "ovl_field_bytes": (C.c_size_t, [_P]),
@@ -44,6 +46,7 @@ SIGNATURES = {
     "ovl_field_export": (_I, [_P, _P, _P]),
     "ovl_dw_native": (_I, [_P, _P, _P]),
     "ovl_overlap_native": (_I, [_P, _D, _I, _P, _P]),
+    "ovl_overlap_multi_native": (_I, [_P, _I, _D, _I, _P, _P]),
     "ovl_set_profiling": (_I, [_P, _I]),
     "ovl_last_poly_timing": (_I, [_P, C.POINTER(C.c_float), C.POINTER(_I)]),
     "ovl_launch_count": (C.c_longlong, [_P]),
@@ -167,6 +170,14 @@ def ovl_sign(ctx, psi, out):
 
 def ovl_overlap(ctx, mu, dagger, psi, out):
     return _check(ctx, load_library().ovl_overlap(ctx, float(mu), int(dagger), _ptr(psi), _ptr(out)))
+
+
+def ovl_overlap_multi(ctx, nrhs, mu, dagger, psi, out):
+    return _check(ctx, load_library().ovl_overlap_multi(ctx, int(nrhs), float(mu), int(dagger), _ptr(psi), _ptr(out)))
+
+
+def ovl_overlap_multi_native(ctx, nrhs, mu, dagger, in_native, out_native):
+    return _check(ctx, load_library().ovl_overlap_multi_native(ctx, int(nrhs), float(mu), int(dagger), _ptr(in_native), _ptr(out_native)))
 
 
 def ovl_cg(ctx, mu, b, x, tol, maxiter):

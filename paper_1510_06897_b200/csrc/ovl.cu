@@ -145,7 +145,8 @@ int ovl_destroy(ovl_ctx *c) {
     if (!c) return OVL_EINVAL;
     cudaStreamSynchronize(c->st);
     void *bufs[] = {c->U, c->phi, c->psi_n, c->out_n, c->tA, c->tB, c->acc, c->g5b, c->cg_r, c->cg_p, c->cg_q, c->cg_Ap,
-                    c->stage_in, c->stage_out, c->proj_partial, c->w_dev, c->coef_dev, c->red_partial, c->sc_dev};
+                    c->stage_in, c->stage_out, c->proj_partial, c->w_dev, c->coef_dev, c->red_partial, c->sc_dev,
+                    c->multi_in, c->multi_out};
     for (void *b : bufs)
         if (b) cudaFree(b);
     for (auto &e : c->graphs)
@@ -219,7 +220,7 @@ int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda
         c->proj_nblk = (int)((c->n() + BLAS_THREADS * PROJ_EPT - 1) / (BLAS_THREADS * PROJ_EPT));
         OVL_CUDA(c, cudaMalloc(&c->phi, c->field_bytes() * nev));
         OVL_CUDA(c, cudaMalloc((void **)&c->proj_partial, sizeof(double2) * (size_t)c->proj_nblk * nev));
-        OVL_CUDA(c, cudaMalloc((void **)&c->w_dev, sizeof(double2) * nev));
+        OVL_CUDA(c, cudaMalloc((void **)&c->w_dev, sizeof(double2) * nev * OVL_MAX_RHS));
         OVL_CUDA(c, cudaMalloc((void **)&c->coef_dev, sizeof(double) * nev));
         c->proj_cap = nev;
     }
@@ -248,7 +249,7 @@ int ovl_khat(ovl_ctx *c, const void *psi, void *out) {
     return with_canonical(c, psi, out, [&](const void *i, void *o) { return DISPATCH(c, khat_native, c, i, o); });
 }
 int ovl_sign(ovl_ctx *c, const void *psi, void *out) {
-    return with_canonical(c, psi, out, [&](const void *i, void *o) { return DISPATCH(c, sign_combine_native, c, 0.0, 1.0, 0, 0, i, o); });
+    return with_canonical(c, psi, out, [&](const void *i, void *o) { return DISPATCH(c, sign_combine_native, c, 1, 0.0, 1.0, 0, 0, i, o); });
 }
 int ovl_overlap(ovl_ctx *c, double mu, int dagger, const void *psi, void *out) {
     return with_canonical(c, psi, out, [&](const void *i, void *o) { return DISPATCH(c, overlap_native, c, mu, dagger ? 1 : 0, i, o); });
@@ -285,6 +286,35 @@ int ovl_dw_native(ovl_ctx *c, const void *in, void *out) {
 int ovl_overlap_native(ovl_ctx *c, double mu, int dagger, const void *in, void *out) {
     if (!c || !in || !out || in == out) return OVL_EINVAL;
     return DISPATCH(c, overlap_native, c, mu, dagger ? 1 : 0, in, out);
+}
+
+int ovl_overlap_multi_native(ovl_ctx *c, int nrhs, double mu, int dagger, const void *in, void *out) {
+    if (!c || !in || !out || in == out) return OVL_EINVAL;
+    if (nrhs < 1 || nrhs > OVL_MAX_RHS) return fail(c, OVL_EINVAL, "nrhs must be in 1..%d", OVL_MAX_RHS);
+    return DISPATCH(c, overlap_native, c, mu, dagger ? 1 : 0, in, out, nrhs);
+}
+
+int ovl_overlap_multi(ovl_ctx *c, int nrhs, double mu, int dagger, const void *psi, void *out) {
+    if (!c) return OVL_EINVAL;
+    if (!psi || !out || psi == out) return fail(c, OVL_EINVAL, "null or aliased spinor pointers");
+    if (nrhs < 1 || nrhs > OVL_MAX_RHS) return fail(c, OVL_EINVAL, "nrhs must be in 1..%d", OVL_MAX_RHS);
+    if (nrhs > c->multi_cap) {
+        OVL_CUDA(c, cudaStreamSynchronize(c->st));
+        if (c->multi_in) cudaFree(c->multi_in);
+        if (c->multi_out) cudaFree(c->multi_out);
+        c->multi_in = c->multi_out = nullptr;
+        c->multi_cap = 0;
+        OVL_TRY(dev_alloc(c, &c->multi_in, c->field_bytes() * nrhs));
+        OVL_TRY(dev_alloc(c, &c->multi_out, c->field_bytes() * nrhs));
+        c->multi_cap = nrhs;
+    }
+    const size_t cb = c->canon_bytes(), fb = c->field_bytes();
+    for (int r = 0; r < nrhs; ++r)
+        OVL_TRY(import_any(c, (const char *)psi + r * cb, (char *)c->multi_in + r * fb));
+    OVL_TRY(DISPATCH(c, overlap_native, c, mu, dagger ? 1 : 0, c->multi_in, c->multi_out, nrhs));
+    for (int r = 0; r < nrhs; ++r)
+        OVL_TRY(export_any(c, (const char *)c->multi_out + r * fb, (char *)out + r * cb));
+    return OVL_OK;
 }
 
 int ovl_set_profiling(ovl_ctx *c, int on) {

@@ -28,6 +28,9 @@ struct ovl_ctx {
     void *U = nullptr;    // links
     void *phi = nullptr;  // eigenvectors [nev][12][V]
     void *psi_n = nullptr, *out_n = nullptr, *tA = nullptr, *tB = nullptr, *acc = nullptr, *g5b = nullptr;
+    int work_nrhs = 1;                               // right-hand sides tA, tB, acc, g5b are sized for
+    void *multi_in = nullptr, *multi_out = nullptr;  // native staging of ovl_overlap_multi (multi_cap fields each)
+    int multi_cap = 0;
     void *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr, *cg_Ap = nullptr;
     void *stage_in = nullptr, *stage_out = nullptr;  // canonical staging for host pointers (12V complex128 each)
     double2 *proj_partial = nullptr, *w_dev = nullptr;
@@ -40,6 +43,7 @@ struct ovl_ctx {
     struct PolyGraph {
         const void *src = nullptr;
         unsigned long long gen = 0, last_use = 0;
+        int nrhs = 1;
         cudaGraphExec_t exec = nullptr;
     };
     static constexpr int NGRAPH = 8;

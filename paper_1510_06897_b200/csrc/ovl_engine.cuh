@@ -24,13 +24,14 @@ struct WilsonArgs {
     const void *in = nullptr, *prev = nullptr, *psi = nullptr;
     void *out = nullptr, *acc = nullptr;
     double c_diag = 0, c_hop = 0, a_psi = 0, a_acc = 0, a_init = 0;
-    int flip = 0;
+    int flip = 0, nrhs = 1;
 };
 
 template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx *c, const WilsonArgs &a) {
     constexpr int TH = WilsonCfg<T>::THREADS;
-    const int grid = (c->g.V + TH - 1) / TH;
-    StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip};
+    const int grid = ((c->g.V + TH - 1) / TH) * a.nrhs;
+    StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip,
+                     a.nrhs, c->n()};
     k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
         c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp);
 }
@@ -57,16 +58,18 @@ template <typename T> int khat_native(ovl_ctx *c, const void *in, void *out) {
 
 // acc = sum_{m=0}^{N} alpha_m T_m(K^) src by the forward recurrence exactly as printed:
 // t_0 = src, t_1 = K^ src, t_{m+1} = 2 K^ t_m - t_{m-1}, acc = sum alpha_m t_m.  N launches.
-template <typename T> int cheb_forward(ovl_ctx *c, const void *src) {
+template <typename T> int cheb_forward(ovl_ctx *c, const void *src, int nrhs) {
     const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
     const std::vector<double> &al = c->alpha;
     const int N = c->norders;
     WilsonArgs a;
+    a.nrhs = nrhs;
     a.in = src; a.out = c->tA; a.acc = c->acc; a.c_diag = cd; a.c_hop = ch; a.a_init = al[0]; a.a_acc = al[1];
     if (N == 1) OVL_TRY((launch_wilson<T, K_G5 | K_ACCI | K_NOWRITE>(c, a)));
     else OVL_TRY((launch_wilson<T, K_G5 | K_ACCI>(c, a)));
     for (int m = 1; m < N; ++m) {  // produces t_{m+1}
         WilsonArgs b;
+        b.nrhs = nrhs;
         b.in = (m & 1) ? c->tA : c->tB;
         b.out = (m & 1) ? c->tB : c->tA;
         b.prev = (m == 1) ? src : b.out;
@@ -84,13 +87,14 @@ template <typename T> int cheb_forward(ovl_ctx *c, const void *src) {
 // acc = alpha_0 src + K^ b_1 - b_2.  It has no read-modify-write accumulator stream: one order reads b_{k+1} (stencil),
 // b_{k+2} and - when alpha_k != 0 - src, and writes b_k over b_{k+2}.  b_N = alpha_N src is never formed: the first
 // launch applies 2 alpha_N K^ to src directly and the second one carries the (- alpha_N src) term.  N launches.
-template <typename T> int cheb_clenshaw(ovl_ctx *c, const void *src) {
+template <typename T> int cheb_clenshaw(ovl_ctx *c, const void *src, int nrhs) {
     const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
     const std::vector<double> &al = c->alpha;
     const int N = c->norders;
     int nl = 0;
     auto step = [&](const void *in, const void *prev, void *out, double scale, double a_psi) -> int {
         WilsonArgs a;
+        a.nrhs = nrhs;
         a.in = in; a.prev = prev; a.psi = src; a.out = out;
         a.c_diag = scale * cd; a.c_hop = scale * ch; a.a_psi = a_psi; a.flip = (nl++) & 1;
         if (prev) return a_psi != 0.0 ? launch_wilson<T, K_G5 | K_PREV | K_PSI>(c, a) : launch_wilson<T, K_G5 | K_PREV>(c, a);
@@ -108,21 +112,21 @@ template <typename T> int cheb_clenshaw(ovl_ctx *c, const void *src) {
     return step(cur, oth, c->acc, 1.0, al[0]);
 }
 
-template <typename T> int cheb_launches(ovl_ctx *c, const void *src) {
-    return c->recurrence == OVL_REC_FORWARD ? cheb_forward<T>(c, src) : cheb_clenshaw<T>(c, src);
+template <typename T> int cheb_launches(ovl_ctx *c, const void *src, int nrhs) {
+    return c->recurrence == OVL_REC_FORWARD ? cheb_forward<T>(c, src, nrhs) : cheb_clenshaw<T>(c, src, nrhs);
 }
 
 // The loop is a fixed sequence of launches for a given source field, so it is captured once into a CUDA graph and
 // replayed (0.5 us instead of 2 us of launch overhead per order on B200: 20 % of an order at 8^3x32).  Capture needs a
 // real stream: on the legacy default stream (handle 0), or if capture fails (the caller is itself capturing), the
 // launches are issued directly.  Returns OVL_OK with *done = false when the caller has to launch directly.
-template <typename T> int cheb_graph(ovl_ctx *c, const void *src, bool *done) {
+template <typename T> int cheb_graph(ovl_ctx *c, const void *src, int nrhs, bool *done) {
     *done = false;
     if (!c->use_graphs || c->st == nullptr || c->st == cudaStreamLegacy || c->st == cudaStreamPerThread) return OVL_OK;
     ovl_ctx::PolyGraph *hit = nullptr, *victim = nullptr;
     for (auto &e : c->graphs) {
         const bool valid = e.exec && e.gen == c->poly_gen;
-        if (valid && e.src == src) hit = &e;
+        if (valid && e.src == src && e.nrhs == nrhs) hit = &e;
         if (!valid) { if (!victim || (victim->exec && victim->gen == c->poly_gen)) victim = &e; }
         else if (!victim || (victim->exec && victim->gen == c->poly_gen && e.last_use < victim->last_use)) victim = &e;
     }
@@ -131,7 +135,7 @@ template <typename T> int cheb_graph(ovl_ctx *c, const void *src, bool *done) {
         if (cudaStreamIsCapturing(c->st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return OVL_OK; }
         if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return OVL_OK; }
         const long long l0 = c->launches;
-        const int rc = cheb_launches<T>(c, src);
+        const int rc = cheb_launches<T>(c, src, nrhs);
         c->launches = l0;  // counted per replay below
         cudaGraph_t gr = nullptr;
         const cudaError_t e = cudaStreamEndCapture(c->st, &gr);
@@ -145,7 +149,7 @@ template <typename T> int cheb_graph(ovl_ctx *c, const void *src, bool *done) {
         cudaGraphDestroy(gr);
         if (ei != cudaSuccess) { cudaGetLastError(); return OVL_OK; }
         if (victim->exec) cudaGraphExecDestroy(victim->exec);
-        victim->exec = ex; victim->src = src; victim->gen = c->poly_gen;
+        victim->exec = ex; victim->src = src; victim->gen = c->poly_gen; victim->nrhs = nrhs;
         hit = victim;
     }
     hit->last_use = ++c->use_clock;
@@ -156,11 +160,11 @@ template <typename T> int cheb_graph(ovl_ctx *c, const void *src, bool *done) {
 }
 
 // acc = sum_{m=0}^{norders} alpha_m T_m(K^) src    (first sum of eq. 2.3; src is not modified)
-template <typename T> int cheb_native(ovl_ctx *c, const void *src) {
+template <typename T> int cheb_native(ovl_ctx *c, const void *src, int nrhs) {
     if (c->profiling) OVL_CUDA(c, cudaEventRecord(c->ev0, c->st));
     bool done = false;
-    OVL_TRY(cheb_graph<T>(c, src, &done));
-    if (!done) OVL_TRY(cheb_launches<T>(c, src));
+    OVL_TRY(cheb_graph<T>(c, src, nrhs, &done));
+    if (!done) OVL_TRY(cheb_launches<T>(c, src, nrhs));
     if (c->profiling) {
         OVL_CUDA(c, cudaEventRecord(c->ev1, c->st));
         c->last_poly_launches = c->norders;
@@ -183,34 +187,57 @@ inline int refresh_coef(ovl_ctx *c) {
     return OVL_OK;
 }
 
-// out = a*in + b*[gamma5]( sign(K) src ),  src = in (dagger = 0) or gamma5 in (dagger = 1, gamma5 not applied on the way out)
-// a = b = ... chosen by the caller: ovl_sign uses a = 0, b = 1, g5out = 0.
-template <typename T> int sign_combine_native(ovl_ctx *c, double a, double b, int dagger, int g5out, const void *in, void *out) {
+// work vectors of the recurrence (t_A, t_B, acc, gamma5 psi) for `nrhs` right-hand sides; grown on demand
+inline int ensure_work(ovl_ctx *c, int nrhs) {
+    if (nrhs <= c->work_nrhs) return OVL_OK;
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    void **bufs[] = {&c->tA, &c->tB, &c->acc, &c->g5b};
+    for (void **b : bufs) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+        OVL_TRY(dev_alloc(c, b, c->field_bytes() * nrhs));
+    }
+    c->work_nrhs = nrhs;
+    ++c->poly_gen;  // captured graphs point at the old buffers
+    return OVL_OK;
+}
+
+// out_r = a*in_r + b*[gamma5]( sign(K) src_r ) for r < nrhs consecutive native fields;  src = in (dagger = 0) or gamma5 in
+// (dagger = 1, gamma5 not applied on the way out).  ovl_sign uses a = 0, b = 1, g5out = 0.  The polynomial loop handles
+// all right-hand sides in every launch (links amortised); the deflation passes run per right-hand side.
+template <typename T> int sign_combine_native(ovl_ctx *c, int nrhs, double a, double b, int dagger, int g5out, const void *in, void *out) {
     if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
+    OVL_TRY(ensure_work(c, nrhs));
     const size_t n = c->n(), n_upper = (size_t)6 * c->g.V;
     const void *src = in;
     if (dagger) {
-        k_gamma5<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(n, n_upper, (const cx<T> *)in, (cx<T> *)c->g5b);
-        OVL_LAUNCH_CHECK(c);
+        for (int r = 0; r < nrhs; ++r) {
+            k_gamma5<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(n, n_upper, (const cx<T> *)in + r * n, (cx<T> *)c->g5b + r * n);
+            OVL_LAUNCH_CHECK(c);
+        }
         src = c->g5b;
     }
     if (c->nev > 0) {
         OVL_TRY(refresh_coef(c));
-        k_project<T><<<c->proj_nblk, BLAS_THREADS, 0, c->st>>>(n, c->nev, (const cx<T> *)c->phi, (const cx<T> *)src, c->proj_partial);
-        OVL_LAUNCH_CHECK(c);
-        k_project_final<<<c->nev, BLAS_THREADS, 0, c->st>>>(c->proj_nblk, c->proj_partial, c->coef_dev, c->w_dev);
+        for (int r = 0; r < nrhs; ++r) {
+            k_project<T><<<c->proj_nblk, BLAS_THREADS, 0, c->st>>>(n, c->nev, (const cx<T> *)c->phi, (const cx<T> *)src + r * n, c->proj_partial);
+            OVL_LAUNCH_CHECK(c);
+            k_project_final<<<c->nev, BLAS_THREADS, 0, c->st>>>(c->proj_nblk, c->proj_partial, c->coef_dev, c->w_dev + (size_t)r * c->proj_cap);
+            OVL_LAUNCH_CHECK(c);
+        }
+    }
+    OVL_TRY(cheb_native<T>(c, src, nrhs));
+    for (int r = 0; r < nrhs; ++r) {
+        k_deflate_assemble<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(
+            n, n_upper, c->nev, (const cx<T> *)c->phi, c->w_dev + (size_t)r * c->proj_cap, (const cx<T> *)in + r * n,
+            (const cx<T> *)c->acc + r * n, (T)a, (T)b, g5out, (cx<T> *)out + r * n);
         OVL_LAUNCH_CHECK(c);
     }
-    OVL_TRY(cheb_native<T>(c, src));
-    k_deflate_assemble<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(
-        n, n_upper, c->nev, (const cx<T> *)c->phi, c->w_dev, (const cx<T> *)in, (const cx<T> *)c->acc, (T)a, (T)b, g5out,
-        (cx<T> *)out);
-    OVL_LAUNCH_CHECK(c);
     return OVL_OK;
 }
 
-template <typename T> int overlap_native(ovl_ctx *c, double mu, int dagger, const void *in, void *out) {
-    return sign_combine_native<T>(c, 0.5 * (1.0 + mu), 0.5 * (1.0 - mu), dagger, dagger ? 0 : 1, in, out);
+template <typename T> int overlap_native(ovl_ctx *c, double mu, int dagger, const void *in, void *out, int nrhs = 1) {
+    return sign_combine_native<T>(c, nrhs, 0.5 * (1.0 + mu), 0.5 * (1.0 - mu), dagger, dagger ? 0 : 1, in, out);
 }
 
 // ---- CG on A = D^dag D (a9).  b_n, x_n native; x0 = 0.

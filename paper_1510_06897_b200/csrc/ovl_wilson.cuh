@@ -42,6 +42,8 @@ enum : int { K_G5 = 1, K_PREV = 2, K_PSI = 4, K_ACC = 8, K_ACCI = 16, K_NOWRITE 
 template <typename T> struct StepParams {
     T c_hop, r_c, r_p, r_a, a_acc, a_init;
     int flip;
+    int nrhs;        // right-hand sides processed by this launch; field r starts at r * fstride
+    size_t fstride;  // complex elements between consecutive right-hand sides (12 V)
 };
 
 // Load the 3x3 link U_mu(su) (rows r, cols c) from the native planes; rebuild row 2 for 12-real storage.
@@ -149,9 +151,25 @@ template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *__restrict__ prev,
                const cx<T> *__restrict__ psi, cx<T> *__restrict__ out, cx<T> *__restrict__ acc, const StepParams<T> sp) {
-    const int tile = sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    // blockIdx.x = rhs + nrhs * tile: the CTAs that work on the same tile for different right-hand sides are adjacent in
+    // launch order, so they run at the same time and the tile's links come from DRAM once and from L2 after that
+    int rhs = 0, ntile = gridDim.x, tile = blockIdx.x;
+    if (sp.nrhs > 1) {
+        rhs = blockIdx.x % sp.nrhs;
+        ntile = gridDim.x / sp.nrhs;
+        tile = blockIdx.x / sp.nrhs;
+    }
+    if (sp.flip) tile = ntile - 1 - tile;
     const int s = tile * THREADS + threadIdx.x;
     if (s >= g.V) return;
+    {
+        const size_t off = (size_t)rhs * sp.fstride;
+        in += off;
+        if (FLAGS & K_PREV) prev += off;
+        if (FLAGS & K_PSI) psi += off;
+        if (!(FLAGS & K_NOWRITE)) out += off;
+        if (FLAGS & (K_ACC | K_ACCI)) acc += off;
+    }
     const int x = s % g.L[0];
     const int y = (s / g.L[0]) % g.L[1];
     const int z = (s / g.sxy) % g.L[2];

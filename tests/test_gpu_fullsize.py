@@ -69,6 +69,23 @@ def test_low_degree_deflated_overlap_vs_oracle_full_size(torch, api, orc, rough,
     assert rel_err(got, want) < 1e-10
 
 
+def test_multi_rhs_full_size_matches_single(torch, api, rough):
+    """4 right-hand sides at 20^3 x 64 in the launch configuration bench.py times (grid = 4 x 4000 CTAs): bit-identical
+    to four single applies (which the tests above pin to the oracle and to the FFT closed form)."""
+    U, psi = rough
+    alpha = inputs.chebyshev_sign_coeffs(12, 0.3)
+    phi = inputs.phase_vectors(DIMS, 2, inputs.SEED_BASE + 204)
+    lam = np.array([0.5, -0.51])
+    with api.Overlap(DIMS, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        p0 = dev(torch, psi)
+        ps = torch.stack([p0, p0.conj().contiguous(), (1j * p0), p0.flip(0).contiguous()])
+        got = op.overlap_multi(ps, 0.01)
+        for r in range(4):
+            assert torch.equal(got[r], op.overlap(ps[r].contiguous(), 0.01)), r
+
+
 @pytest.mark.parametrize("prec,tol,rec", [("f64", 1e-10, "clenshaw"), ("f64", 1e-10, "forward"), ("f32", 1e-5, "clenshaw"),
                                           ("f32", 1e-5, "forward")])
 def test_degree400_sign_vs_fft_closed_form_full_size(torch, api, prec, tol, rec):

@@ -325,6 +325,56 @@ def test_graph_replay_equals_direct_launches(torch, api, orc, rec):
     assert rel_err(res[True][4], orc.sign(dims, U, a2, psi, m_w=1.4, lambda_max=6.2)) < TOL_OVL
 
 
+@pytest.mark.parametrize("prec,tol", [("f64", TOL_OVL), ("f32", TOL_F32)])
+@pytest.mark.parametrize("rec", RECS)
+@pytest.mark.parametrize("nrhs,dagger", [(1, False), (3, False), (5, True), (12, False)])
+def test_multi_rhs_overlap(torch, api, orc, prec, tol, rec, nrhs, dagger):
+    """ovl_overlap_multi: every right-hand side against the oracle, and bit-identical to the
+    single-right-hand-side call (same arithmetic per site; only the CTA -> (tile, rhs) map differs)."""
+    dims = (4, 6, 8, 10)   # 1920 sites = 15 tiles of 128
+    nev = 4
+    U = inputs.config_links(dims, 0.3, 51, stout_steps=1)
+    phi = inputs.orthonormal_vectors(dims, nev, 52)
+    lam = np.array([0.31, -0.33, 0.35, -0.4])
+    alpha = inputs.chebyshev_sign_coeffs(21, 0.2)
+    psis = np.stack([inputs.gaussian_spinor(dims, 60 + r) for r in range(nrhs)])
+    cd = torch.complex128 if prec == "f64" else torch.complex64
+    with api.Overlap(dims, dev(torch, U), prec) as op:
+        op.set_recurrence(rec)
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        p = dev(torch, psis, cd)
+        got = op.overlap_multi(p, 0.02, dagger=dagger)
+        singles = torch.stack([op.overlap(p[r].contiguous(), 0.02, dagger=dagger) for r in range(nrhs)])
+        assert torch.equal(got, singles)
+        again = op.overlap_multi(p, 0.02, dagger=dagger)       # workspace already grown, graph replay on side streams
+        assert torch.equal(got, again)
+    got = host(got)
+    for r in range(nrhs):
+        want = orc.overlap(dims, U, alpha, 0.02, psis[r], phi, lam, dagger=dagger)
+        assert rel_err(got[r].astype(np.complex128), want) < tol, r
+
+
+def test_multi_rhs_host_pointers_and_errors(torch, api, orc):
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 4, 6)
+    U = inputs.random_links(dims, 0.4, 71)
+    alpha = rough_alpha(9, seed=2)
+    psis = np.stack([inputs.gaussian_spinor(dims, 80 + r) for r in range(2)])
+    with api.Overlap(dims, U) as op:            # host links
+        with pytest.raises(B.OvlError) as e:
+            op.overlap_multi(psis, 0.1)          # no polynomial yet
+        assert e.value.code == B.OVL_ESTATE
+        op.set_chebyshev(alpha)
+        got = op.overlap_multi(psis, 0.1)        # numpy in, numpy out: staged by the library
+        for r in range(2):
+            assert rel_err(got[r], orc.overlap(dims, U, alpha, 0.1, psis[r])) < TOL_OVL
+        out = np.empty_like(psis)
+        for bad in (0, B.OVL_MAX_RHS + 1):
+            rc = B.load_library().ovl_overlap_multi(op.ctx, bad, 0.1, 0, B._ptr(psis), B._ptr(out))
+            assert rc == B.OVL_EINVAL
+
+
 def test_bit_identical_run_to_run(torch, api):
     dims = (6, 6, 6, 10)
     U = dev(torch, inputs.random_links(dims, 0.4, 61))
