@@ -192,10 +192,17 @@ inline int ensure_work(ovl_ctx *c, int nrhs) {
     if (nrhs <= c->work_nrhs) return OVL_OK;
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     void **bufs[] = {&c->tA, &c->tB, &c->acc, &c->g5b};
-    for (void **b : bufs) {
-        if (*b) cudaFree(*b);
-        *b = nullptr;
-        OVL_TRY(dev_alloc(c, b, c->field_bytes() * nrhs));
+    void *fresh[4] = {nullptr, nullptr, nullptr, nullptr};
+    for (int i = 0; i < 4; ++i) {
+        const int rc = dev_alloc(c, &fresh[i], c->field_bytes() * nrhs);
+        if (rc != OVL_OK) {  // keep the old (smaller) workspace usable
+            for (int j = 0; j < i; ++j) cudaFree(fresh[j]);
+            return rc;
+        }
+    }
+    for (int i = 0; i < 4; ++i) {
+        if (*bufs[i]) cudaFree(*bufs[i]);
+        *bufs[i] = fresh[i];
     }
     c->work_nrhs = nrhs;
     ++c->poly_gen;  // captured graphs point at the old buffers

@@ -72,6 +72,17 @@ def random_links(dims, eps: float, seed: int) -> np.ndarray:
     return np.ascontiguousarray(_exp_i_hermitian(h, eps))
 
 
+def tiled_links(dims, block, eps: float, seed: int) -> np.ndarray:
+    """random_links on a `block` sub-lattice, repeated periodically to fill `dims` (every extent of dims a multiple of
+    the block's).  Still a valid SU(3) gauge field; used where generating V*4 independent matrices on the host would
+    take minutes (the 48^3 x 96 volume of BASELINE config 4)."""
+    reps = [d // b for d, b in zip(dims, block)]
+    assert all(r * b == d for r, b, d in zip(reps, block, dims)), "dims must be multiples of block"
+    u = _lat(random_links(block, eps, seed), block)                       # (bt, bz, by, bx, 4, 3, 3)
+    u = np.tile(u, (reps[3], reps[2], reps[1], reps[0], 1, 1, 1))
+    return np.ascontiguousarray(u.reshape(volume(dims), 4, 3, 3))
+
+
 def random_su3_field(dims, seed: int, eps: float = 2.0) -> np.ndarray:
     """One SU(3) matrix g(x) per site, far from identity; shape (V, 3, 3). For gauge transformations."""
     h = _traceless_hermitian(_rng(seed), (volume(dims),))
