@@ -232,22 +232,39 @@ def time_region(torch, stream, fn, steps, dist=None):
     return ms
 
 
-def dslash_sweep_point(torch, api, dims, prec, recon, reps=100):
-    """Standalone D_W on native fields: sites/s, compulsory-bytes GB/s (2S + 4L per site) and requested-bytes GB/s."""
-    U = inputs.random_links(dims, 0.3, inputs.SEED_BASE + 4)
-    psi = inputs.gaussian_spinor(dims, inputs.SEED_BASE + 104)
-    pb = 8 if prec == "f64" else 4
-    with api.Overlap(dims, torch.from_numpy(U).cuda(), prec, recon) as op:
-        p = torch.from_numpy(psi).cuda().to(op.cdtype)
-        a, b = op.to_native(p), op.native_empty()
-        for _ in range(5):
-            op.dw_native(a, b)
-        ms = time_region(torch, op.stream, lambda: op.dw_native(a, b), reps) / reps
-    V = int(np.prod(dims))
-    S, L = 24 * pb, recon * pb
-    return {"dims": "x".join(map(str, dims)), "prec": prec, "recon": recon, "us": 1e3 * ms,
-            "gsites_per_s": V / ms / 1e6, "gbs_compulsory": V * (2 * S + 4 * L) / ms / 1e6,
-            "gbs_requested": V * (9 * S + 8 * L) / ms / 1e6}
+SWEEP_VOLUMES = [  # (dims, block the links are tiled from): the metric's two sizes, then BASELINE config 4
+    ((8, 8, 8, 32), (8, 8, 8, 32)), ((20, 20, 20, 64), (20, 20, 20, 64)),
+    ((8, 8, 8, 8), (8, 8, 8, 8)), ((16, 16, 16, 32), (8, 8, 8, 16)), ((24, 24, 24, 48), (12, 12, 12, 24)),
+    ((32, 32, 32, 64), (8, 8, 8, 16)), ((48, 48, 48, 96), (12, 12, 12, 24)),
+]
+
+
+def dslash_sweep(torch, api, hbm_peak, reps=100):
+    """Standalone D_W on native fields (BASELINE config 4 + the metric's 8^3x32 and 20^3x64): sites/s, compulsory-bytes
+    GB/s (2S + 4L per site) and requested-bytes GB/s, fp64/fp32 x 18/12-real links.  Links: seeded random near-identity
+    SU(3) (eps = 0.3), tiled from a sub-block for the big volumes (inputs.tiled_links); spinors Gaussian."""
+    out = []
+    for dims, block in SWEEP_VOLUMES:
+        U = inputs.tiled_links(dims, block, 0.3, inputs.SEED_BASE + 4)
+        psi = inputs.gaussian_spinor(dims, inputs.SEED_BASE + 104)
+        V = int(np.prod(dims))
+        for prec, recon in [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)]:
+            pb = 8 if prec == "f64" else 4
+            with api.Overlap(dims, U, prec, recon) as op:
+                p = torch.from_numpy(psi).cuda().to(op.cdtype)
+                a, b = op.to_native(p), op.native_empty()
+                del p
+                for _ in range(5):
+                    op.dw_native(a, b)
+                n = reps if V < 4_000_000 else 30
+                ms = time_region(torch, op.stream, lambda: op.dw_native(a, b), n) / n
+            S, L = 24 * pb, recon * pb
+            out.append({"dims": "x".join(map(str, dims)), "prec": prec, "recon": recon, "us": 1e3 * ms,
+                        "gsites_per_s": V / ms / 1e6, "gbs_compulsory": V * (2 * S + 4 * L) / ms / 1e6,
+                        "gbs_requested": V * (9 * S + 8 * L) / ms / 1e6,
+                        "frac_of_measured_peak": V * (2 * S + 4 * L) / ms / 1e6 / hbm_peak})
+        del U, psi
+    return out
 
 
 def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with_e2e, host_inputs=None,
@@ -422,13 +439,7 @@ def run_native(args, w):
             extras[f"cfg3_{other}_recurrence"] = {
                 "applies_per_s": ro["applies_per_s"], "achieved_gbs": ro["achieved_gbs"], "frac": ro["achieved_gbs"] / hbm_peak,
                 "kernel_us": ro["kernel_us"], "algorithmic_bytes_per_site_per_launch": ro["bytes_per_site_per_order"]}
-        sweep = []
-        for dims in [(8, 8, 8, 32), (20, 20, 20, 64)]:
-            for prec, recon in [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)]:
-                pt = dslash_sweep_point(torch, api, dims, prec, recon)
-                pt["frac_of_measured_peak"] = pt["gbs_compulsory"] / hbm_peak
-                sweep.append(pt)
-        extras["dslash"] = sweep
+        extras["dslash"] = dslash_sweep(torch, api, hbm_peak)
         U, psi, alpha, phi, lam = host_inputs
         r, cores, desc, _ = oracle_overlap_rate(w, U, psi, alpha, phi, lam, args.ref_orders)
         line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
