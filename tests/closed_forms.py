@@ -85,3 +85,34 @@ def free_sign_fft(dims, psi, gammas, m_w=1.5, g=None):
     if g is not None:
         out = np.einsum("xab,xsb->xsa", g, out)
     return out, omega
+
+
+def lowest_pure_gauge_eigenpairs(dims, g, gammas, nev, m_w=1.5):
+    """Exact eigenpairs of K = gamma5 (D_W - m_w) on the pure gauge U_mu(x) = g(x) g(x+mu)^dag (g = None: U = 1), the
+    `nev` of smallest |lambda| (ties cut in a fixed order, R11): K[U^g] = g K[1] g^dag site by site, and on
+    U = 1 the plane wave exp(i p.x) u e_c is an eigenvector whenever u is an eigenvector of the Hermitian 4x4 symbol
+    gamma5 ((4 - m_w - sum cos p) + i sum gamma_mu sin p), eigenvalues +-omega(p), each twice, times 3 colours.
+    Returns (phi of shape (nev, V, 4, 3), orthonormal; lambda of shape (nev,))."""
+    lx, ly, lz, lt = dims
+    v = lx * ly * lz * lt
+    px, py, pz, pt = momenta(dims)
+    a = 4.0 - m_w - (np.cos(px) + np.cos(py) + np.cos(pz) + np.cos(pt))
+    om = np.sqrt(a * a + np.sin(px) ** 2 + np.sin(py) ** 2 + np.sin(pz) ** 2 + np.sin(pt) ** 2 + 0 * a).reshape(-1)
+    order = np.argsort(om, kind="stable")
+    g5 = np.diag([1.0, 1.0, -1.0, -1.0]).astype(np.complex128)
+    gm = np.eye(3, dtype=np.complex128)[None].repeat(v, 0) if g is None else g
+    phis, lams = [], []
+    for flat in order:
+        nt, rem = divmod(int(flat), lz * ly * lx)
+        nz, rem = divmod(rem, ly * lx)
+        ny, nx = divmod(rem, lx)
+        wave, p = plane_wave(dims, (nx, ny, nz, nt), np.ones((1, 1)))
+        ph = wave[:, 0, 0] / np.sqrt(v)
+        lam, vec = np.linalg.eigh(g5 @ dw_symbol(p, gammas, m_w))
+        for j in np.argsort(np.abs(lam), kind="stable"):
+            for c in range(3):
+                phis.append(ph[:, None, None] * vec[:, j][None, :, None] * gm[:, None, :, c])
+                lams.append(lam[j])
+                if len(phis) == nev:
+                    return np.ascontiguousarray(np.stack(phis)), np.array(lams)
+    raise ValueError("nev exceeds 12 V")

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from paper_1510_06897_b200 import inputs
-from tests.closed_forms import free_sign_fft, golden_gammas
+from tests.closed_forms import free_sign_fft, golden_gammas, lowest_pure_gauge_eigenpairs
 from tests.conftest import rel_err
 
 pytestmark = pytest.mark.gpu
@@ -131,3 +131,29 @@ def test_degree400_sign_vs_fft_closed_form_full_size(torch, api, prec, tol, rec)
         side.synchronize()
     assert rel_err(got, exact) < tol
     assert rel_err(s2, psi) < 2 * tol  # sign(K)^2 = 1
+
+
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_config3_true_eigenpairs_degree400_nev50_full_size(torch, api, prec, tol):
+    """BASELINE config 3 exactly as named -- 20^3 x 64, mu = 0.01, degree 400, 50 deflated eigenpairs -- with TRUE
+    eigenpairs: the closed-form lowest modes of K on a pure gauge.  D[mu] psi against the FFT closed form (the polynomial's
+    error on this spectrum is < 1e-11), plus sign(K) phi_i = sign(lambda_i) phi_i on two of the deflated modes."""
+    U, g = inputs.pure_gauge_links(DIMS, inputs.SEED_BASE + 34)
+    G = golden_gammas()
+    phi, lam = lowest_pure_gauge_eigenpairs(DIMS, g, G, 50)
+    psi = inputs.gaussian_spinor(DIMS, inputs.SEED_BASE + 134)
+    exact, omega = free_sign_fft(DIMS, psi, G, 1.5, g)
+    alpha = inputs.chebyshev_sign_coeffs(400, 0.95 * omega.min() / 6.5)
+    assert np.abs(inputs.chebyshev_eval(alpha, omega.ravel() / 6.5) - 1.0).max() < 1e-11
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+    want = 0.5 * (1.01 * psi + 0.99 * g5 * exact)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side), api.Overlap(DIMS, dev(torch, U), prec, stream=side) as op:
+        assert op.set_chebyshev(alpha) == 399
+        op.set_deflation(dev(torch, phi), lam)
+        got = op.overlap(dev(torch, psi, op.cdtype), 0.01).cpu().numpy().astype(np.complex128)
+        e = [op.sign(dev(torch, phi[i], op.cdtype)).cpu().numpy().astype(np.complex128) for i in (0, 49)]
+        side.synchronize()
+    assert rel_err(got, want) < tol
+    for i, ei in zip((0, 49), e):
+        assert rel_err(ei, np.sign(lam[i]) * phi[i]) < (1e-12 if prec == "f64" else tol)

@@ -375,6 +375,33 @@ def test_multi_rhs_host_pointers_and_errors(torch, api, orc):
             assert rc == B.OVL_EINVAL
 
 
+@pytest.mark.parametrize("prec,tol", [("f64", TOL_OVL), ("f32", TOL_F32)])
+def test_config1_true_eigenpairs_pure_gauge_8x8x8x32(torch, api, orc, prec, tol):
+    """BASELINE config 1 with TRUE eigenpairs: 8^3 x 32, degree 200, the 20 lowest-|lambda| eigenpairs of K in closed form
+    on a pure gauge (gauge-rotated plane waves, tests/closed_forms.py; pinned against the oracle's K in the CPU suite).
+    Tier A against the oracle, Tier B against the FFT closed form, and sign(K) phi_i = sign(lambda_i) phi_i."""
+    from tests.closed_forms import free_sign_fft, golden_gammas, lowest_pure_gauge_eigenpairs
+    dims, nev = (8, 8, 8, 32), 20
+    U, g = inputs.pure_gauge_links(dims, inputs.SEED_BASE + 31)
+    G = golden_gammas()
+    phi, lam = lowest_pure_gauge_eigenpairs(dims, g, G, nev)
+    psi = inputs.gaussian_spinor(dims, inputs.SEED_BASE + 131)
+    exact, omega = free_sign_fft(dims, psi, G, 1.5, g)
+    alpha = inputs.chebyshev_sign_coeffs(200, 0.95 * omega.min() / 6.5)
+    delta = np.abs(inputs.chebyshev_eval(alpha, omega.ravel() / 6.5) - 1.0).max()
+    want = orc.overlap(dims, U, alpha, 0.01, psi, phi, lam)
+    with api.Overlap(dims, dev(torch, U), prec) as op:
+        assert op.set_chebyshev(alpha) == 199
+        op.set_deflation(dev(torch, phi), lam)
+        p = dev(torch, psi, op.cdtype)
+        got = host(op.overlap(p, 0.01)).astype(np.complex128)
+        s = host(op.sign(p)).astype(np.complex128)
+        e7 = host(op.sign(dev(torch, phi[7], op.cdtype))).astype(np.complex128)
+    assert rel_err(got, want) < tol                                       # Tier A
+    assert rel_err(s, exact) < max(2 * delta, tol)                        # Tier B (delta ~ 5e-8 at N = 200)
+    assert rel_err(e7, np.sign(lam[7]) * phi[7]) < (1e-12 if prec == "f64" else tol)
+
+
 def test_bit_identical_run_to_run(torch, api):
     dims = (6, 6, 6, 10)
     U = dev(torch, inputs.random_links(dims, 0.4, 61))

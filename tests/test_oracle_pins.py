@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from paper_1510_06897_b200 import inputs
-from tests.closed_forms import dw_symbol, free_sign_fft, golden_gammas, plane_wave
+from tests.closed_forms import dw_symbol, free_sign_fft, golden_gammas, lowest_pure_gauge_eigenpairs, plane_wave
 from tests.conftest import rel_err
 
 G5 = np.array([1.0, 1.0, -1.0, -1.0])
@@ -347,3 +347,32 @@ def test_links_unitary_and_smearing_raises_plaquette():
     assert np.abs(a - b).max() < 1e-12
     Upg, _ = inputs.pure_gauge_links(dims, 8)
     assert abs(inputs.plaquette(Upg, dims) - 1) < 1e-13
+
+
+def test_deflation_with_closed_form_eigenpairs_pure_gauge(orc):
+    """eq. 2.3 with TRUE eigenpairs at a volume with no dense matrix: on a pure gauge the lowest eigenpairs of K are
+    gauge-rotated plane waves (tests/closed_forms.py).  (i) the oracle's K reproduces them; (ii) with them deflated,
+    sign(K) phi_i = sign(lambda_i) phi_i to rounding even with a deliberately poor polynomial, while without deflation
+    the error is the polynomial's |1 - p(lambda^_i)|; (iii) on a random psi the deflated sum is within the polynomial's
+    error on the REST of the spectrum of the FFT closed form."""
+    dims, nev = (4, 4, 6, 8), 24
+    U, g = inputs.pure_gauge_links(dims, 51)
+    G = golden_gammas()
+    phi, lam = lowest_pure_gauge_eigenpairs(dims, g, G, nev)
+    for i in (0, 7, 23):
+        assert np.linalg.norm(orc.khat(dims, U, phi[i], 1.5, 6.5) * 6.5 - lam[i] * phi[i]) < 1e-13
+    alpha = inputs.chebyshev_sign_coeffs(11, 0.3)          # poor on purpose: |lambda^| ~ 0.09 < eps = 0.3
+    perr = np.abs(inputs.chebyshev_eval(alpha, np.abs(lam) / 6.5) - 1.0)
+    assert perr.min() > 0.05
+    for i in (0, 11, 23):
+        with_defl = orc.sign(dims, U, alpha, phi[i], phi, lam)
+        without = orc.sign(dims, U, alpha, phi[i])
+        assert np.linalg.norm(with_defl - np.sign(lam[i]) * phi[i]) < 1e-13
+        assert abs(np.linalg.norm(without - np.sign(lam[i]) * phi[i]) - perr[i]) < 1e-10
+    psi = inputs.gaussian_spinor(dims, 52)
+    exact, omega = free_sign_fft(dims, psi, G, 1.5, g)
+    rest = np.sort(omega.ravel())[nev // 12:]              # |lambda| of the modes that are not deflated (12 per momentum)
+    alpha = inputs.chebyshev_sign_coeffs(81, 0.95 * rest.min() / 6.5)
+    delta = np.abs(inputs.chebyshev_eval(alpha, rest / 6.5) - 1.0).max()
+    got = orc.sign(dims, U, alpha, psi, phi, lam)
+    assert np.linalg.norm(got - exact) <= 1.05 * delta * np.linalg.norm(psi) + 1e-12
