@@ -369,6 +369,25 @@ def bench_cg(torch, api, w, steps_tol=1e-8):
             "applies_per_s": applies / dt, "us_per_order": 1e6 * dt / (applies * orders)}
 
 
+def bench_cg_multi(torch, api, w, nrhs=12, tol=1e-8):
+    """The propagator workload: nrhs = 12 sources solved in lockstep with ovl_cg_multi on the config-2
+    lattice; seconds per solved system against the single-system CG of bench_cg."""
+    U, b, alpha, phi, lam = make_inputs(w, seed_off=7)
+    bs = np.stack([inputs.gaussian_spinor(w["dims"], inputs.SEED_BASE + 300 + r) for r in range(nrhs)])
+    with api.Overlap(w["dims"], torch.from_numpy(U).cuda()) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(torch.from_numpy(phi).cuda(), lam)
+        bd = torch.from_numpy(bs).cuda()
+        op.cg_multi(bd, 0.05, tol=0.0, maxiter=1)  # warm-up (workspace growth, graph capture)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        x, its, rels, ok = op.cg_multi(bd, 0.05, tol=tol, maxiter=2000)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+    return {"nrhs": nrhs, "iterations": its, "max_true_relres": max(rels), "converged": ok, "seconds": dt,
+            "seconds_per_system": dt / nrhs}
+
+
 def run_native(args, w):
     import torch
 
@@ -426,6 +445,7 @@ def run_native(args, w):
             extras["cfg1_8x8x8x32"] = {"applies_per_s": r1["applies_per_s"], "us_per_order": r1["kernel_us"],
                                         "orders": r1["orders"]}
             extras["cfg2_cg"] = bench_cg(torch, api, w1)
+            extras["cfg2_cg_12rhs"] = bench_cg_multi(torch, api, w1)
             extras["multi_rhs"] = {
                 "cfg3_20x20x20x64_fp64_4rhs": bench_multi(torch, api, w, "f64", args.recon, 4, 2, 2, host_inputs),
                 "cfg1_8x8x8x32_fp64_12rhs": bench_multi(torch, api, w1, "f64", 18, 12, 10, 3)}

@@ -130,6 +130,13 @@ int ovl_overlap_multi(ovl_ctx *ctx, int nrhs, double mu, int dagger, const void 
 int ovl_cg(ovl_ctx *ctx, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out,
            double *true_relres_out);
 
+/* nrhs independent systems D^dag D x_r = b_r solved in lockstep (1 <= nrhs <= OVL_MAX_RHS): every operator application
+ * is one multi-right-hand-side call (see ovl_overlap_multi), alpha, beta and the residual norms are kept per system; a
+ * system that has reached tol is frozen while the others iterate.  b, x [H|D]: [nrhs][V][4][3]; iters_out, true_relres_out:
+ * host arrays of nrhs entries.  Returns OVL_ENOTCONV if any system is above tol after maxiter iterations.  Synchronises. */
+int ovl_cg_multi(ovl_ctx *ctx, int nrhs, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out,
+                 double *true_relres_out);
+
 const char *ovl_last_error(const ovl_ctx *ctx);
 
 /* ---- native-layout fields (benchmark / solver plumbing: no relayout passes inside the timed calls) -------------

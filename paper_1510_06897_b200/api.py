@@ -102,6 +102,12 @@ class Overlap:
         rc, it, rel = B.ovl_cg(self.ctx, mu, b, x, tol, maxiter)
         return x, it, rel, rc == B.OVL_OK
 
+    def cg_multi(self, b, mu, tol=1e-8, maxiter=1000):
+        """b: (nrhs, V, 4, 3). Solve D^dag D x_r = b_r in lockstep. Returns (x, iterations[], true relres[], converged)."""
+        x = self._like(b)
+        rc, it, rel = B.ovl_cg_multi(self.ctx, int(b.shape[0]), mu, b, x, tol, maxiter)
+        return x, it, rel, rc == B.OVL_OK
+
     # ---- native-layout fields
     def native_empty(self, nrhs=1):
         torch = _torch()

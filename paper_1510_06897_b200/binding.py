@@ -40,6 +40,7 @@ SIGNATURES = {
     "ovl_overlap": (_I, [_P, _D, _I, _P, _P]),
     "ovl_overlap_multi": (_I, [_P, _I, _D, _I, _P, _P]),
     "ovl_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_cg_multi": (_I, [_P, _I, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_last_error": (C.c_char_p, [_P]),
     "ovl_field_bytes": (C.c_size_t, [_P]),
     "ovl_field_import": (_I, [_P, _P, _P]),
@@ -186,6 +187,14 @@ def ovl_cg(ctx, mu, b, x, tol, maxiter):
     rc = load_library().ovl_cg(ctx, float(mu), _ptr(b), _ptr(x), float(tol), int(maxiter), C.byref(it), C.byref(rel))
     _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
     return rc, int(it.value), float(rel.value)
+
+
+def ovl_cg_multi(ctx, nrhs, mu, b, x, tol, maxiter):
+    """Returns (status, iterations per system, true relative residual per system)."""
+    it, rel = (_I * nrhs)(), (_D * nrhs)()
+    rc = load_library().ovl_cg_multi(ctx, int(nrhs), float(mu), _ptr(b), _ptr(x), float(tol), int(maxiter), it, rel)
+    _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, list(it), list(rel)
 
 
 def ovl_last_error(ctx) -> str:

@@ -111,10 +111,10 @@ int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int pre
         void **bufs[] = {&c->psi_n, &c->out_n, &c->tA, &c->tB, &c->acc, &c->g5b};
         for (void **b : bufs) OVL_TRY(dev_alloc(c, b, fb));
         c->red_nblk = grid_for(c->n(), BLAS_THREADS * 4, 148 * 8);
-        OVL_CUDA(c, cudaMalloc((void **)&c->red_partial, sizeof(double) * c->red_nblk));
-        OVL_CUDA(c, cudaMalloc((void **)&c->sc_dev, sizeof(double) * SC_N));
-        OVL_CUDA(c, cudaMemsetAsync(c->sc_dev, 0, sizeof(double) * SC_N, c->st));
-        OVL_CUDA(c, cudaMallocHost((void **)&c->sc_host, sizeof(double) * SC_N));
+        OVL_CUDA(c, cudaMalloc((void **)&c->red_partial, sizeof(double) * c->red_nblk * OVL_MAX_RHS));
+        OVL_CUDA(c, cudaMalloc((void **)&c->sc_dev, sizeof(double) * SC_N * OVL_MAX_RHS));
+        OVL_CUDA(c, cudaMemsetAsync(c->sc_dev, 0, sizeof(double) * SC_N * OVL_MAX_RHS, c->st));
+        OVL_CUDA(c, cudaMallocHost((void **)&c->sc_host, sizeof(double) * SC_N * OVL_MAX_RHS));
         OVL_CUDA(c, cudaMalloc((void **)&c->w_dev, sizeof(double2)));
         OVL_CUDA(c, cudaEventCreate(&c->ev0));
         OVL_CUDA(c, cudaEventCreate(&c->ev1));
@@ -264,6 +264,33 @@ int ovl_cg(ovl_ctx *c, double mu, const void *b, void *x, double tol, int maxite
     if (rc != OVL_OK && rc != OVL_ENOTCONV) return rc;
     int rc2 = export_any(c, c->out_n, x);
     if (rc2 != OVL_OK) return rc2;
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    return rc;
+}
+
+int ovl_cg_multi(ovl_ctx *c, int nrhs, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out, double *relres_out) {
+    if (!c) return OVL_EINVAL;
+    if (!b || !x || b == x || !iters_out || !relres_out || maxiter < 0) return fail(c, OVL_EINVAL, "bad ovl_cg_multi arguments");
+    if (nrhs < 1 || nrhs > OVL_MAX_RHS) return fail(c, OVL_EINVAL, "nrhs must be in 1..%d", OVL_MAX_RHS);
+    if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
+    if (nrhs > c->multi_cap) {
+        OVL_CUDA(c, cudaStreamSynchronize(c->st));
+        if (c->multi_in) cudaFree(c->multi_in);
+        if (c->multi_out) cudaFree(c->multi_out);
+        c->multi_in = c->multi_out = nullptr;
+        c->multi_cap = 0;
+        OVL_TRY(dev_alloc(c, &c->multi_in, c->field_bytes() * nrhs));
+        OVL_TRY(dev_alloc(c, &c->multi_out, c->field_bytes() * nrhs));
+        c->multi_cap = nrhs;
+    }
+    const size_t cb = c->canon_bytes(), fb = c->field_bytes();
+    for (int r = 0; r < nrhs; ++r) OVL_TRY(import_any(c, (const char *)b + r * cb, (char *)c->multi_in + r * fb));
+    int rc = DISPATCH(c, cg_native, c, mu, c->multi_in, c->multi_out, tol, maxiter, iters_out, relres_out, nrhs);
+    if (rc != OVL_OK && rc != OVL_ENOTCONV) return rc;
+    for (int r = 0; r < nrhs; ++r) {
+        int rc2 = export_any(c, (const char *)c->multi_out + r * fb, (char *)x + r * cb);
+        if (rc2 != OVL_OK) return rc2;
+    }
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     return rc;
 }

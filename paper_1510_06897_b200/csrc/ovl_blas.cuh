@@ -150,14 +150,17 @@ __global__ void k_gamma5(size_t n, size_t n_upper, const cx<T> *__restrict__ in,
 }
 
 // ---------------------------------------------------------------- a9: CG vector kernels (device-side scalars)
-// sc[]: 0 rr, 1 pAp, 2 alpha, 3 beta, 4 bb
-enum { SC_RR = 0, SC_PAP = 1, SC_ALPHA = 2, SC_BETA = 3, SC_BB = 4, SC_N = 8 };
+// sc[]: 0 rr, 1 pAp, 2 alpha, 3 beta, 4 bb, 5 frozen (system reached the tolerance: alpha = beta = 0 from then on)
+// Batched over right-hand sides with blockIdx.y = rhs: field r starts at r*n, its scalars at r*SC_N, its partial sums
+// at r*gridDim.x (gridDim.y = 1 is the single-system CG).
+enum { SC_RR = 0, SC_PAP = 1, SC_ALPHA = 2, SC_BETA = 3, SC_BB = 4, SC_FROZEN = 5, SC_N = 8 };
 
 // partial[b] = sum Re(conj(x) y) over the block's grid-stride elements
 template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS)
 k_redot(size_t n, const cx<T> *__restrict__ x, const cx<T> *__restrict__ y, double *__restrict__ partial) {
     __shared__ double sm[BLAS_THREADS / 32];
+    x += blockIdx.y * n; y += blockIdx.y * n; partial += blockIdx.y * gridDim.x;
     double r = 0;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const cx<T> a = x[e], b = y[e];
@@ -172,6 +175,8 @@ __global__ void __launch_bounds__(BLAS_THREADS)
 k_cg_update(size_t n, const double *__restrict__ sc, const cx<T> *__restrict__ p, const cx<T> *__restrict__ q,
             cx<T> *__restrict__ x, cx<T> *__restrict__ r, double *__restrict__ partial) {
     __shared__ double sm[BLAS_THREADS / 32];
+    p += blockIdx.y * n; q += blockIdx.y * n; x += blockIdx.y * n; r += blockIdx.y * n;
+    sc += blockIdx.y * SC_N; partial += blockIdx.y * gridDim.x;
     const T al = (T)sc[SC_ALPHA];
     double acc = 0;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
@@ -188,6 +193,7 @@ k_cg_update(size_t n, const double *__restrict__ sc, const cx<T> *__restrict__ p
 // p = r + beta p   (beta = sc[SC_BETA])
 template <typename T>
 __global__ void k_xpay(size_t n, const double *__restrict__ sc, const cx<T> *__restrict__ r, cx<T> *__restrict__ p) {
+    r += blockIdx.y * n; p += blockIdx.y * n; sc += blockIdx.y * SC_N;
     const T be = (T)sc[SC_BETA];
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const cx<T> re = r[e];
@@ -199,23 +205,35 @@ __global__ void k_xpay(size_t n, const double *__restrict__ sc, const cx<T> *__r
 // out = x - y  (true residual)
 template <typename T>
 __global__ void k_sub(size_t n, const cx<T> *__restrict__ x, const cx<T> *__restrict__ y, cx<T> *__restrict__ out) {
+    x += blockIdx.y * n; y += blockIdx.y * n; out += blockIdx.y * n;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const cx<T> a = x[e], b = y[e];
         out[e] = mk<T>(a.x - b.x, a.y - b.y);
     }
 }
-// second stage of the CG reductions, one block.  what: 0 -> bb = rr = sum (start), 1 -> pAp = sum, alpha = rr / pAp,
-// 2 -> rr_new = sum, beta = rr_new / rr, rr = rr_new, 3 -> sc[SC_PAP] = sum (generic norm^2 read-out)
-__global__ void __launch_bounds__(BLAS_THREADS) k_cg_scalars(int nblk, const double *__restrict__ partial, double *sc, int what) {
+// second stage of the CG reductions, one block per system (blockIdx.x = rhs).  what: 0 -> bb = rr = sum (start),
+// 1 -> pAp = sum, alpha = rr / pAp (0 if frozen), 2 -> rr_new = sum, beta = rr_new / rr, rr = rr_new; the system is
+// frozen once rr_new <= tol2 * bb (tol2 = 0: never), 3 -> sc[SC_PAP] = sum (generic norm^2 read-out)
+__global__ void __launch_bounds__(BLAS_THREADS)
+k_cg_scalars(int nblk, const double *__restrict__ partial, double *sc, int what, double tol2) {
     __shared__ double sm[BLAS_THREADS / 32];
+    partial += (size_t)blockIdx.x * nblk;
+    sc += blockIdx.x * SC_N;
     double r = 0;
     for (int b = threadIdx.x; b < nblk; b += blockDim.x) r += partial[b];
     r = block_sum(r, sm);
     if (threadIdx.x == 0) {
-        if (what == 0) { sc[SC_BB] = r; sc[SC_RR] = r; }
-        else if (what == 1) { sc[SC_PAP] = r; sc[SC_ALPHA] = sc[SC_RR] / r; }
-        else if (what == 2) { sc[SC_BETA] = r / sc[SC_RR]; sc[SC_RR] = r; }
-        else { sc[SC_PAP] = r; }
+        const bool frozen = sc[SC_FROZEN] != 0.0;
+        if (what == 0) { sc[SC_BB] = r; sc[SC_RR] = r; sc[SC_FROZEN] = 0.0; sc[SC_ALPHA] = 0.0; sc[SC_BETA] = 0.0; }
+        else if (what == 1) { sc[SC_PAP] = r; sc[SC_ALPHA] = frozen ? 0.0 : sc[SC_RR] / r; }
+        else if (what == 2) {
+            if (frozen) sc[SC_BETA] = 0.0;
+            else {
+                sc[SC_BETA] = r / sc[SC_RR];
+                sc[SC_RR] = r;
+                if (tol2 > 0.0 && r <= tol2 * sc[SC_BB]) { sc[SC_FROZEN] = 1.0; sc[SC_BETA] = 0.0; }
+            }
+        } else { sc[SC_PAP] = r; }
     }
 }
 

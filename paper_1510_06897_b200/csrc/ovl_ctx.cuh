@@ -32,6 +32,7 @@ struct ovl_ctx {
     void *multi_in = nullptr, *multi_out = nullptr;  // native staging of ovl_overlap_multi (multi_cap fields each)
     int multi_cap = 0;
     void *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr, *cg_Ap = nullptr;
+    int cg_nrhs = 0;  // systems the CG vectors are sized for
     void *stage_in = nullptr, *stage_out = nullptr;  // canonical staging for host pointers (12V complex128 each)
     double2 *proj_partial = nullptr, *w_dev = nullptr;
     double *coef_dev = nullptr;

@@ -247,62 +247,94 @@ template <typename T> int overlap_native(ovl_ctx *c, double mu, int dagger, cons
     return sign_combine_native<T>(c, nrhs, 0.5 * (1.0 + mu), 0.5 * (1.0 - mu), dagger, dagger ? 0 : 1, in, out);
 }
 
-// ---- CG on A = D^dag D (a9).  b_n, x_n native; x0 = 0.
-template <typename T> int reduce_redot(ovl_ctx *c, const void *x, const void *y, int what) {
-    k_redot<T><<<c->red_nblk, BLAS_THREADS, 0, c->st>>>(c->n(), (const cx<T> *)x, (const cx<T> *)y, c->red_partial);
+// ---- CG on A = D^dag D (a9), nrhs independent systems in lockstep (nrhs = 1: the plain CG).  b_n, x_n: nrhs
+// consecutive native fields; x0 = 0.  Every operator application handles all systems at once (multi-right-hand-side
+// kernel launches); the vector kernels are batched over blockIdx.y with per-system alpha, beta, rr on the device.  A
+// system that reaches the tolerance is frozen (alpha = beta = 0: x and r stop changing) while the others go on.
+template <typename T> int reduce_redot(ovl_ctx *c, const void *x, const void *y, int what, int nrhs) {
+    k_redot<T><<<dim3(c->red_nblk, nrhs), BLAS_THREADS, 0, c->st>>>(c->n(), (const cx<T> *)x, (const cx<T> *)y, c->red_partial);
     OVL_LAUNCH_CHECK(c);
-    k_cg_scalars<<<1, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, what);
+    k_cg_scalars<<<nrhs, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, what, 0.0);
     OVL_LAUNCH_CHECK(c);
     return OVL_OK;
 }
-inline int fetch_scalars(ovl_ctx *c) {
-    OVL_CUDA(c, cudaMemcpyAsync(c->sc_host, c->sc_dev, sizeof(double) * SC_N, cudaMemcpyDeviceToHost, c->st));
+inline int fetch_scalars(ovl_ctx *c, int nrhs) {
+    OVL_CUDA(c, cudaMemcpyAsync(c->sc_host, c->sc_dev, sizeof(double) * SC_N * nrhs, cudaMemcpyDeviceToHost, c->st));
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    return OVL_OK;
+}
+inline int ensure_cg(ovl_ctx *c, int nrhs) {
+    if (nrhs <= c->cg_nrhs) return OVL_OK;
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    void **bufs[] = {&c->cg_r, &c->cg_p, &c->cg_q, &c->cg_Ap};
+    for (void **b : bufs) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+    }
+    c->cg_nrhs = 0;
+    for (void **b : bufs) OVL_TRY(dev_alloc(c, b, c->field_bytes() * nrhs));
+    c->cg_nrhs = nrhs;
     return OVL_OK;
 }
 
 template <typename T>
-int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int maxiter, int *iters, double *relres) {
-    const size_t n = c->n(), fb = c->field_bytes();
-    OVL_TRY(dev_alloc(c, &c->cg_r, fb));
-    OVL_TRY(dev_alloc(c, &c->cg_p, fb));
-    OVL_TRY(dev_alloc(c, &c->cg_q, fb));
-    OVL_TRY(dev_alloc(c, &c->cg_Ap, fb));
+int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int maxiter, int *iters, double *relres, int nrhs = 1) {
+    const size_t n = c->n(), fb = c->field_bytes() * nrhs;
+    OVL_TRY(ensure_cg(c, nrhs));
     OVL_CUDA(c, cudaMemsetAsync(x_n, 0, fb, c->st));
     OVL_CUDA(c, cudaMemcpyAsync(c->cg_r, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
     OVL_CUDA(c, cudaMemcpyAsync(c->cg_p, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
-    OVL_TRY(reduce_redot<T>(c, b_n, b_n, 0));
-    OVL_TRY(fetch_scalars(c));
-    const double bb = c->sc_host[SC_BB];
-    double rr = bb;
+    OVL_TRY(reduce_redot<T>(c, b_n, b_n, 0, nrhs));
+    OVL_TRY(fetch_scalars(c, nrhs));
+    double bb[OVL_MAX_RHS], rr[OVL_MAX_RHS];
+    bool conv[OVL_MAX_RHS];
+    const double tol2 = tol > 0 ? tol * tol : 0.0;
+    int nconv = 0;
+    for (int r = 0; r < nrhs; ++r) {
+        bb[r] = rr[r] = c->sc_host[r * SC_N + SC_BB];
+        iters[r] = 0;
+        conv[r] = tol > 0 && rr[r] <= tol2 * bb[r];  // b = 0
+        nconv += conv[r];
+    }
     int it = 0;
-    const int gridv = grid_for(n, BLAS_THREADS);
-    while (it < maxiter && !(tol > 0 && std::sqrt(rr) <= tol * std::sqrt(bb))) {
-        OVL_TRY(overlap_native<T>(c, mu, 0, c->cg_p, c->cg_q));
-        OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap));
-        OVL_TRY(reduce_redot<T>(c, c->cg_p, c->cg_Ap, 1));  // alpha = rr / Re(p^dag A p)
-        k_cg_update<T><<<c->red_nblk, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_p, (const cx<T> *)c->cg_Ap,
-                                                               (cx<T> *)x_n, (cx<T> *)c->cg_r, c->red_partial);
+    const dim3 gridv(grid_for(n, BLAS_THREADS), nrhs), gridr(c->red_nblk, nrhs);
+    while (it < maxiter && nconv < nrhs) {
+        OVL_TRY(overlap_native<T>(c, mu, 0, c->cg_p, c->cg_q, nrhs));
+        OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap, nrhs));
+        OVL_TRY(reduce_redot<T>(c, c->cg_p, c->cg_Ap, 1, nrhs));  // alpha = rr / Re(p^dag A p)
+        k_cg_update<T><<<gridr, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_p, (const cx<T> *)c->cg_Ap,
+                                                        (cx<T> *)x_n, (cx<T> *)c->cg_r, c->red_partial);
         OVL_LAUNCH_CHECK(c);
-        k_cg_scalars<<<1, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, 2);  // beta, rr
+        // beta, rr; with several systems the converged ones are frozen on the device (a single system just stops)
+        k_cg_scalars<<<nrhs, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, 2, nrhs > 1 ? tol2 : 0.0);
         OVL_LAUNCH_CHECK(c);
         k_xpay<T><<<gridv, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_r, (cx<T> *)c->cg_p);
         OVL_LAUNCH_CHECK(c);
-        OVL_TRY(fetch_scalars(c));  // the convergence scalar is the only host round trip per iteration
-        rr = c->sc_host[SC_RR];
+        OVL_TRY(fetch_scalars(c, nrhs));  // the convergence scalars are the only host round trip per iteration
         ++it;
-        if (!(rr == rr)) return fail(c, OVL_ECUDA, "CG broke down (NaN residual) at iteration %d", it);
+        for (int r = 0; r < nrhs; ++r) {
+            if (conv[r]) continue;
+            rr[r] = c->sc_host[r * SC_N + SC_RR];
+            iters[r] = it;
+            if (!(rr[r] == rr[r])) return fail(c, OVL_ECUDA, "CG broke down (NaN residual) at iteration %d, system %d", it, r);
+            if (tol > 0 && rr[r] <= tol2 * bb[r]) { conv[r] = true; ++nconv; }  // same test as the device-side freeze
+        }
     }
-    // true residual ||b - A x|| / ||b||
-    OVL_TRY(overlap_native<T>(c, mu, 0, x_n, c->cg_q));
-    OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap));
+    // true residuals ||b - A x|| / ||b||
+    OVL_TRY(overlap_native<T>(c, mu, 0, x_n, c->cg_q, nrhs));
+    OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap, nrhs));
     k_sub<T><<<gridv, BLAS_THREADS, 0, c->st>>>(n, (const cx<T> *)b_n, (const cx<T> *)c->cg_Ap, (cx<T> *)c->cg_q);
     OVL_LAUNCH_CHECK(c);
-    OVL_TRY(reduce_redot<T>(c, c->cg_q, c->cg_q, 3));
-    OVL_TRY(fetch_scalars(c));
-    *iters = it;
-    *relres = std::sqrt(c->sc_host[SC_PAP] / bb);
-    if (tol > 0 && !(std::sqrt(rr) <= tol * std::sqrt(bb))) return fail(c, OVL_ENOTCONV, "CG: %d iterations, ||r||/||b|| = %.3e > tol", it, std::sqrt(rr / bb));
+    OVL_TRY(reduce_redot<T>(c, c->cg_q, c->cg_q, 3, nrhs));
+    OVL_TRY(fetch_scalars(c, nrhs));
+    for (int r = 0; r < nrhs; ++r) relres[r] = bb[r] > 0 ? std::sqrt(c->sc_host[r * SC_N + SC_PAP] / bb[r]) : 0.0;
+    if (tol > 0 && nconv < nrhs) {
+        int worst = 0;
+        for (int r = 1; r < nrhs; ++r)
+            if (rr[r] / bb[r] > rr[worst] / bb[worst]) worst = r;
+        return fail(c, OVL_ENOTCONV, "CG: %d iterations, %d of %d systems above tol (worst ||r||/||b|| = %.3e, system %d)", it,
+                    nrhs - nconv, nrhs, std::sqrt(rr[worst] / bb[worst]), worst);
+    }
     return OVL_OK;
 }
 

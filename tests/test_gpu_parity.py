@@ -355,6 +355,40 @@ def test_multi_rhs_overlap(torch, api, orc, prec, tol, rec, nrhs, dagger):
         assert rel_err(got[r].astype(np.complex128), want) < tol, r
 
 
+def test_cg_multi_lockstep(torch, api, orc):
+    """ovl_cg_multi: 3 systems with very different right-hand sides (one is a constant vector that converges at a
+    different iteration and must be frozen).  Each solution is bit-identical to the single-system ovl_cg, iteration
+    counts agree, true residuals <= tol; a fixed-iteration run matches the oracle CG at 1e-10."""
+    dims = (4, 4, 4, 8)
+    U = inputs.config_links(dims, 0.3, 77, stout_steps=1)
+    alpha = inputs.chebyshev_sign_coeffs(41, 0.09)
+    phi = inputs.orthonormal_vectors(dims, 3, 78)
+    lam = np.array([0.45, -0.47, 0.5])
+    b = np.stack([inputs.gaussian_spinor(dims, 79), 1e-3 * inputs.gaussian_spinor(dims, 80), inputs.gaussian_spinor(dims, 81)])
+    b[2] = b[2] * 0 + 1.0          # constant vector: a different (smaller) Krylov space
+    mu = 0.2
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        bd = dev(torch, b)
+        x, its, rels, ok = op.cg_multi(bd, mu, tol=1e-9, maxiter=500)
+        assert ok and len(its) == 3
+        for r in range(3):
+            xs, it1, rel1, ok1 = op.cg(bd[r].contiguous(), mu, tol=1e-9, maxiter=500)
+            assert ok1 and it1 == its[r]
+            assert torch.equal(xs, x[r])
+            assert rels[r] <= 1.05e-9 and abs(rels[r] - rel1) <= 1e-12
+        assert len(set(its)) > 1       # they did not all stop together: freezing was exercised
+        x5, its5, _, _ = op.cg_multi(bd, mu, tol=0.0, maxiter=5)
+        assert its5 == [5, 5, 5]
+        xnc, itn, reln, okn = op.cg_multi(bd, mu, tol=1e-9, maxiter=3)
+        assert not okn and itn == [3, 3, 3]
+    x5 = host(x5)
+    for r in range(3):
+        xo, _, _ = orc.cg(dims, U, alpha, mu, b[r], 0.0, 5, phi, lam)
+        assert rel_err(x5[r], xo) < TOL_OVL
+
+
 def test_multi_rhs_host_pointers_and_errors(torch, api, orc):
     from paper_1510_06897_b200 import binding as B
     dims = (4, 4, 4, 6)
