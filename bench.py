@@ -388,6 +388,33 @@ def bench_cg_multi(torch, api, w, nrhs=12, tol=1e-8):
             "seconds_per_system": dt / nrhs}
 
 
+def bench_cg_mixed(torch, api, w, host_inputs=None, tol=1e-8, inner_tol=1e-4, label=""):
+    """fp32 inner / fp64 outer CG (ovl_cg_mixed) against the all-fp64 ovl_cg on the same system."""
+    U, b, alpha, phi, lam = host_inputs if host_inputs is not None else make_inputs(w, seed_off=7)
+    Ud = torch.from_numpy(U).cuda()
+    with api.Overlap(w["dims"], Ud, "f64") as op, api.Overlap(w["dims"], Ud, "f32") as op32:
+        for o in (op, op32):
+            o.set_chebyshev(alpha)
+            if w["nev"]:
+                phid = torch.from_numpy(phi).cuda()
+                o.set_deflation(phid, lam)
+                del phid
+        bd = torch.from_numpy(b).cuda()
+        op.cg_mixed(op32, bd, 0.05, tol=1e-1, inner_tol=1e-1, max_outer=1, max_inner=2)  # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        x, no, ni, rel, ok = op.cg_mixed(op32, bd, 0.05, tol=tol, inner_tol=inner_tol)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        x64, it64, rel64, ok64 = op.cg(bd, 0.05, tol=tol, maxiter=2000)
+        torch.cuda.synchronize()
+        dt64 = time.perf_counter() - t0
+        diff = float(torch.linalg.norm(x - x64) / torch.linalg.norm(x64))
+    return {"workload": label, "mixed_seconds": dt, "outer_steps": no, "fp32_iterations": ni, "true_relres": rel, "converged": ok,
+            "fp64_seconds": dt64, "fp64_iterations": it64, "fp64_true_relres": rel64, "rel_diff_of_solutions": diff}
+
+
 def run_native(args, w):
     import torch
 
@@ -446,6 +473,9 @@ def run_native(args, w):
                                         "orders": r1["orders"]}
             extras["cfg2_cg"] = bench_cg(torch, api, w1)
             extras["cfg2_cg_12rhs"] = bench_cg_multi(torch, api, w1)
+            extras["cfg2_cg_mixed"] = bench_cg_mixed(torch, api, w1, label="config 2 (8^3x32, mu=0.05, tol 1e-8)")
+            extras["cfg3_cg_mixed"] = bench_cg_mixed(torch, api, w, host_inputs,
+                                                     label="config-3 lattice (20^3x64, N=400, 50 vectors), mu=0.05, tol 1e-8")
             extras["multi_rhs"] = {
                 "cfg3_20x20x20x64_fp64_4rhs": bench_multi(torch, api, w, "f64", args.recon, 4, 2, 2, host_inputs),
                 "cfg1_8x8x8x32_fp64_12rhs": bench_multi(torch, api, w1, "f64", 18, 12, 10, 3)}

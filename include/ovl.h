@@ -137,6 +137,18 @@ int ovl_cg(ovl_ctx *ctx, double mu, const void *b, void *x, double tol, int maxi
 int ovl_cg_multi(ovl_ctx *ctx, int nrhs, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out,
                  double *true_relres_out);
 
+/* Mixed-precision CG on D^dag D x = b ("10^-13 for overlap fermions (using mixed precision)"; SURVEY.md
+ * §8(f) rank 2): defect correction x <- x + A32^{-1}(b - A64 x).  ctx64 is an OVL_F64 context and carries b, x (canonical
+ * complex128 [H|D]), the outer fp64 residuals and the final accuracy; ctx32 is an OVL_F32 context on the same lattice and
+ * the same stream, with its own links / Chebyshev table / deflation set (the table may be of lower degree: the paper's
+ * relaxed inner sign function).  Each outer step solves for the unit-normalised residual with the fp32 CG to the relative
+ * tolerance inner_tol (at most max_inner iterations) and recomputes the residual in fp64 (two fp64 applies).  Stops when
+ * ||b - A64 x|| <= tol ||b||, after max_outer steps, or when an outer step no longer lowers the residual.
+ * *outer_out / *inner_total_out = outer steps / fp32 iterations done; *true_relres_out = fp64 ||b - A x|| / ||b||.
+ * Returns OVL_ENOTCONV (x = best iterate) if tol was not reached; OVL_EINVAL for mismatched contexts.  Synchronises. */
+int ovl_cg_mixed(ovl_ctx *ctx64, ovl_ctx *ctx32, double mu, const void *b, void *x, double tol, double inner_tol,
+                 int max_outer, int max_inner, int *outer_out, int *inner_total_out, double *true_relres_out);
+
 const char *ovl_last_error(const ovl_ctx *ctx);
 
 /* ---- native-layout fields (benchmark / solver plumbing: no relayout passes inside the timed calls) -------------

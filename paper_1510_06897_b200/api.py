@@ -108,6 +108,13 @@ class Overlap:
         rc, it, rel = B.ovl_cg_multi(self.ctx, int(b.shape[0]), mu, b, x, tol, maxiter)
         return x, it, rel, rc == B.OVL_OK
 
+    def cg_mixed(self, inner, b, mu, tol=1e-8, inner_tol=1e-4, max_outer=20, max_inner=1000):
+        """Mixed-precision CG: self is the fp64 operator, `inner` an fp32 Overlap on the same lattice and stream.
+        Returns (x, outer steps, fp32 iterations, true fp64 relres, converged)."""
+        x = self._like(b)
+        rc, no, ni, rel = B.ovl_cg_mixed(self.ctx, inner.ctx, mu, b, x, tol, inner_tol, max_outer, max_inner)
+        return x, no, ni, rel, rc == B.OVL_OK
+
     # ---- native-layout fields
     def native_empty(self, nrhs=1):
         torch = _torch()

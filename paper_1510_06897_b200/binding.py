@@ -41,6 +41,7 @@ SIGNATURES = {
     "ovl_overlap_multi": (_I, [_P, _I, _D, _I, _P, _P]),
     "ovl_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_multi": (_I, [_P, _I, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_cg_mixed": (_I, [_P, _P, _D, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
     "ovl_last_error": (C.c_char_p, [_P]),
     "ovl_field_bytes": (C.c_size_t, [_P]),
     "ovl_field_import": (_I, [_P, _P, _P]),
@@ -195,6 +196,15 @@ def ovl_cg_multi(ctx, nrhs, mu, b, x, tol, maxiter):
     rc = load_library().ovl_cg_multi(ctx, int(nrhs), float(mu), _ptr(b), _ptr(x), float(tol), int(maxiter), it, rel)
     _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
     return rc, list(it), list(rel)
+
+
+def ovl_cg_mixed(ctx64, ctx32, mu, b, x, tol, inner_tol, max_outer, max_inner):
+    """Returns (status, outer steps, total fp32 iterations, true fp64 relative residual)."""
+    no, ni, rel = _I(0), _I(0), _D(0.0)
+    rc = load_library().ovl_cg_mixed(ctx64, ctx32, float(mu), _ptr(b), _ptr(x), float(tol), float(inner_tol), int(max_outer),
+                                     int(max_inner), C.byref(no), C.byref(ni), C.byref(rel))
+    _check(ctx64, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, int(no.value), int(ni.value), float(rel.value)
 
 
 def ovl_last_error(ctx) -> str:

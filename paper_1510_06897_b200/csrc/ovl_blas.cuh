@@ -211,6 +211,25 @@ __global__ void k_sub(size_t n, const cx<T> *__restrict__ x, const cx<T> *__rest
         out[e] = mk<T>(a.x - b.x, a.y - b.y);
     }
 }
+// mixed precision (fp32 inner / fp64 outer defect correction): dst = scale * src across precisions, x += scale * e
+template <typename TS, typename TD>
+__global__ void k_convert_scaled(size_t n, double scale, const cx<TS> *__restrict__ src, cx<TD> *__restrict__ dst) {
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const cx<TS> v = src[e];
+        dst[e] = mk<TD>((TD)(scale * (double)v.x), (TD)(scale * (double)v.y));
+    }
+}
+template <typename TE, typename TX>
+__global__ void k_axpy_mixed(size_t n, double scale, const cx<TE> *__restrict__ e_, cx<TX> *__restrict__ x) {
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const cx<TE> v = e_[e];
+        cx<TX> xe = x[e];
+        xe.x = (TX)((double)xe.x + scale * (double)v.x);
+        xe.y = (TX)((double)xe.y + scale * (double)v.y);
+        x[e] = xe;
+    }
+}
+
 // second stage of the CG reductions, one block per system (blockIdx.x = rhs).  what: 0 -> bb = rr = sum (start),
 // 1 -> pAp = sum, alpha = rr / pAp (0 if frozen), 2 -> rr_new = sum, beta = rr_new / rr, rr = rr_new; the system is
 // frozen once rr_new <= tol2 * bb (tol2 = 0: never), 3 -> sc[SC_PAP] = sum (generic norm^2 read-out)

@@ -338,4 +338,55 @@ int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int
     return OVL_OK;
 }
 
+// ---- mixed-precision CG ("10^-13 for overlap fermions (using mixed precision)"):
+// defect correction x <- x + A32^{-1} (b - A64 x).  Outer residuals and the solution are fp64 (context c), the inner
+// solves run the whole fp32 path (context c32: fp32 links, eigenvectors, stencil arithmetic; its own Chebyshev table, which
+// may be of lower degree) on the residual normalised to unit length.  b_n, x_n: native fp64 fields of c.
+inline int cg_mixed_native(ovl_ctx *c, ovl_ctx *c32, double mu, const void *b_n, void *x_n, double tol, double inner_tol,
+                           int max_outer, int max_inner, int *outer_out, int *inner_out, double *relres) {
+    const size_t n = c->n(), fb = c->field_bytes();
+    OVL_TRY(ensure_cg(c, 1));
+    const int gridv = grid_for(n, BLAS_THREADS);
+    OVL_CUDA(c, cudaMemsetAsync(x_n, 0, fb, c->st));
+    OVL_CUDA(c, cudaMemcpyAsync(c->cg_r, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
+    OVL_TRY(reduce_redot<double>(c, b_n, b_n, 0, 1));
+    OVL_TRY(fetch_scalars(c, 1));
+    const double bb = c->sc_host[SC_BB];
+    double rr = bb;
+    int outer = 0, inner_total = 0;
+    while (outer < max_outer && bb > 0 && !(rr <= tol * tol * bb)) {
+        const double rn = std::sqrt(rr);
+        k_convert_scaled<double, float><<<gridv, BLAS_THREADS, 0, c->st>>>(n, 1.0 / rn, (const double2 *)c->cg_r, (float2 *)c32->psi_n);
+        OVL_LAUNCH_CHECK(c);
+        int it = 0;
+        double rel32 = 0;
+        const int rc = cg_native<float>(c32, mu, c32->psi_n, c32->out_n, inner_tol, max_inner, &it, &rel32, 1);
+        if (rc != OVL_OK && rc != OVL_ENOTCONV) return fail(c, rc, "inner fp32 CG: %s", c32->err);
+        inner_total += it;
+        k_axpy_mixed<float, double><<<gridv, BLAS_THREADS, 0, c->st>>>(n, rn, (const float2 *)c32->out_n, (double2 *)x_n);
+        OVL_LAUNCH_CHECK(c);
+        // r = b - A64 x
+        OVL_TRY(overlap_native<double>(c, mu, 0, x_n, c->cg_q));
+        OVL_TRY(overlap_native<double>(c, mu, 1, c->cg_q, c->cg_Ap));
+        k_sub<double><<<gridv, BLAS_THREADS, 0, c->st>>>(n, (const double2 *)b_n, (const double2 *)c->cg_Ap, (double2 *)c->cg_r);
+        OVL_LAUNCH_CHECK(c);
+        OVL_TRY(reduce_redot<double>(c, c->cg_r, c->cg_r, 3, 1));
+        OVL_TRY(fetch_scalars(c, 1));
+        const double rr_new = c->sc_host[SC_PAP];
+        ++outer;
+        if (!(rr_new == rr_new)) return fail(c, OVL_ECUDA, "mixed CG broke down (NaN residual) in outer iteration %d", outer);
+        if (it == 0 || rr_new >= rr) {  // no progress: the fp32 operator cannot improve this residual any further
+            rr = rr_new < rr ? rr_new : rr;
+            break;
+        }
+        rr = rr_new;
+    }
+    *outer_out = outer;
+    *inner_out = inner_total;
+    *relres = bb > 0 ? std::sqrt(rr / bb) : 0.0;  // rr is the TRUE fp64 residual of the returned x
+    if (bb > 0 && !(rr <= tol * tol * bb))
+        return fail(c, OVL_ENOTCONV, "mixed CG: %d outer / %d inner iterations, ||r||/||b|| = %.3e > tol", outer, inner_total, std::sqrt(rr / bb));
+    return OVL_OK;
+}
+
 }  // namespace ovl

@@ -389,6 +389,48 @@ def test_cg_multi_lockstep(torch, api, orc):
         assert rel_err(x5[r], xo) < TOL_OVL
 
 
+def test_cg_mixed_precision(torch, api, orc):
+    """ovl_cg_mixed: fp32 inner solves, fp64 outer residuals.  Reaches a true fp64 residual of 1e-11 -- far below what the
+    fp32 path alone can represent -- and agrees with the oracle's fp64 CG solution (R14: both are solutions to their
+    tolerance; kappa * tol bounds the difference).  Also with a lower-degree ("relaxed") inner polynomial."""
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 4, 8)
+    U = inputs.config_links(dims, 0.3, 177, stout_steps=1)
+    alpha = inputs.chebyshev_sign_coeffs(61, 0.09)
+    alpha_lo = inputs.chebyshev_sign_coeffs(31, 0.09)
+    phi = inputs.orthonormal_vectors(dims, 3, 178)
+    lam = np.array([0.45, -0.47, 0.5])
+    b = inputs.gaussian_spinor(dims, 179)
+    mu = 0.2
+    xo, ito, relo = orc.cg(dims, U, alpha, mu, b, 1e-11, 500, phi, lam)
+    with api.Overlap(dims, dev(torch, U), "f64") as op, api.Overlap(dims, dev(torch, U), "f32") as op32:
+        for o in (op, op32):
+            o.set_chebyshev(alpha)
+            o.set_deflation(dev(torch, phi), lam)
+        bd = dev(torch, b)
+        x, no, ni, rel, ok = op.cg_mixed(op32, bd, mu, tol=1e-11, inner_tol=1e-4)
+        assert ok and rel <= 1e-11 and 2 <= no <= 6 and ni >= ito // 2
+        assert rel_err(host(x), xo) < 1e-8
+        # the residual reported is the true one: recompute it through the public fp64 operator
+        ax = op.overlap(op.overlap(x, mu), mu, dagger=True)
+        assert abs(float(torch.linalg.norm(bd - ax) / torch.linalg.norm(bd)) - rel) < 1e-13
+        # relaxed inner sign function: lower-degree table in the fp32 context only
+        op32.set_chebyshev(alpha_lo)
+        x2, no2, ni2, rel2, ok2 = op.cg_mixed(op32, bd, mu, tol=1e-9, inner_tol=1e-3, max_outer=60)
+        assert ok2 and rel2 <= 1e-9 and rel_err(host(x2), xo) < 1e-6
+        # not converged within the outer budget -> OVL_ENOTCONV, best iterate returned
+        x3, no3, _, rel3, ok3 = op.cg_mixed(op32, bd, mu, tol=1e-12, inner_tol=1e-1, max_outer=1)
+        assert not ok3 and no3 == 1 and rel3 < 1.0
+        # argument checks: wrong precisions, different lattices
+        out = torch.empty_like(bd)
+        with pytest.raises(B.OvlError):
+            B.ovl_cg_mixed(op32.ctx, op.ctx, mu, bd, out, 1e-8, 1e-4, 5, 100)
+        with api.Overlap((4, 4, 4, 4), inputs.random_links((4, 4, 4, 4), 0.3, 1), "f32") as other:
+            other.set_chebyshev(alpha)
+            with pytest.raises(B.OvlError):
+                B.ovl_cg_mixed(op.ctx, other.ctx, mu, bd, out, 1e-8, 1e-4, 5, 100)
+
+
 def test_multi_rhs_host_pointers_and_errors(torch, api, orc):
     from paper_1510_06897_b200 import binding as B
     dims = (4, 4, 4, 6)
