@@ -415,6 +415,19 @@ def bench_cg_mixed(torch, api, w, host_inputs=None, tol=1e-8, inner_tol=1e-4, la
             "fp64_seconds": dt64, "fp64_iterations": it64, "fp64_true_relres": rel64, "rel_diff_of_solutions": diff}
 
 
+def bench_eigensolver(torch, api, w, nev, block, degree):
+    """the deflation space computed on the GPU (ovl_lowest_eigenpairs), wall-clock seconds."""
+    U = make_inputs(w, need_phi=False)[0]
+    with api.Overlap(w["dims"], torch.from_numpy(U).cuda()) as op:
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        phi, lam, res, cyc, ok = op.lowest_eigenpairs(nev, tol=1e-8, filter_degree=degree, block=block)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+    return {"nev": nev, "block": block, "filter_degree": degree, "cycles": cyc, "converged": ok, "seconds": dt,
+            "max_residual": float(res.max()), "abs_lambda_min": float(np.abs(lam).min()), "abs_lambda_max": float(np.abs(lam).max())}
+
+
 def run_native(args, w):
     import torch
 
@@ -472,6 +485,7 @@ def run_native(args, w):
             extras["cfg1_8x8x8x32"] = {"applies_per_s": r1["applies_per_s"], "us_per_order": r1["kernel_us"],
                                         "orders": r1["orders"]}
             extras["cfg2_cg"] = bench_cg(torch, api, w1)
+            extras["cfg1_eigensolver"] = bench_eigensolver(torch, api, w1, 20, 40, 200)
             extras["cfg2_cg_12rhs"] = bench_cg_multi(torch, api, w1)
             extras["cfg2_cg_mixed"] = bench_cg_mixed(torch, api, w1, label="config 2 (8^3x32, mu=0.05, tol 1e-8)")
             extras["cfg3_cg_mixed"] = bench_cg_mixed(torch, api, w, host_inputs,

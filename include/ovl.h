@@ -149,6 +149,20 @@ int ovl_cg_multi(ovl_ctx *ctx, int nrhs, double mu, const void *b, void *x, doub
 int ovl_cg_mixed(ovl_ctx *ctx64, ovl_ctx *ctx32, double mu, const void *b, void *x, double tol, double inner_tol,
                  int max_outer, int max_inner, int *outer_out, int *inner_total_out, double *true_relres_out);
 
+/* The nev eigenpairs of K = gamma5 (D_W - m_w) of smallest |lambda| -- the deflation space of eq. 2.3 (PAPER.md:62, :66:
+ * "a polynomial preconditioned implicitly restarted Lanczos routine"; here a Chebyshev-filtered block subspace iteration on
+ * K^2 with a Rayleigh-Ritz step on K, which separates +lambda from -lambda).  OVL_F64 contexts.
+ *   tol            stop when ||K phi_i - lambda_i phi_i|| <= tol for all i < nev (phi_i normalised)
+ *   max_cycles     filter + Rayleigh-Ritz cycles at most;  filter_degree: Chebyshev degree in K^2 per cycle (0 = 100)
+ *   block          trial vectors (0 = nev + max(8, nev/2); at most 128).  A block that ends inside a cluster of
+ *                  (near-)degenerate eigenvalues converges slowly: choose it to reach past the cluster.
+ *   phi_out [H|D]  nev canonical complex128 spinors [nev][V][4][3], orthonormal; lambda_out, resid_out (may be NULL):
+ *                  host arrays of nev entries, sorted by |lambda|; *cycles_out = cycles done.
+ * Device memory: 3 * block fields on top of the context, released on return.  Deterministic (fixed start vectors).
+ * Returns OVL_ENOTCONV (best Ritz pairs returned) if tol was not reached.  Synchronises. */
+int ovl_lowest_eigenpairs(ovl_ctx *ctx, int nev, double tol, int max_cycles, int filter_degree, int block, void *phi_out,
+                          double *lambda_out, double *resid_out, int *cycles_out);
+
 const char *ovl_last_error(const ovl_ctx *ctx);
 
 /* ---- native-layout fields (benchmark / solver plumbing: no relayout passes inside the timed calls) -------------

@@ -115,6 +115,14 @@ class Overlap:
         rc, no, ni, rel = B.ovl_cg_mixed(self.ctx, inner.ctx, mu, b, x, tol, inner_tol, max_outer, max_inner)
         return x, no, ni, rel, rc == B.OVL_OK
 
+    def lowest_eigenpairs(self, nev, tol=1e-8, max_cycles=40, filter_degree=100, block=0):
+        """Deflation space on the GPU: the nev lowest-|lambda| eigenpairs of K. Returns (phi (nev,V,4,3) complex128 CUDA
+        tensor, lambda, residuals, cycles, converged)."""
+        torch = _torch()
+        phi = torch.empty((nev, self.V, 4, 3), dtype=torch.complex128, device="cuda")
+        rc, lam, res, cyc = B.ovl_lowest_eigenpairs(self.ctx, nev, tol, max_cycles, filter_degree, block, phi)
+        return phi, lam, res, cyc, rc == B.OVL_OK
+
     # ---- native-layout fields
     def native_empty(self, nrhs=1):
         torch = _torch()

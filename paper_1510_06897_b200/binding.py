@@ -42,6 +42,7 @@ SIGNATURES = {
     "ovl_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_multi": (_I, [_P, _I, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_mixed": (_I, [_P, _P, _D, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_lowest_eigenpairs": (_I, [_P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I)]),
     "ovl_last_error": (C.c_char_p, [_P]),
     "ovl_field_bytes": (C.c_size_t, [_P]),
     "ovl_field_import": (_I, [_P, _P, _P]),
@@ -205,6 +206,15 @@ def ovl_cg_mixed(ctx64, ctx32, mu, b, x, tol, inner_tol, max_outer, max_inner):
                                      int(max_inner), C.byref(no), C.byref(ni), C.byref(rel))
     _check(ctx64, rc, ok=(OVL_OK, OVL_ENOTCONV))
     return rc, int(no.value), int(ni.value), float(rel.value)
+
+
+def ovl_lowest_eigenpairs(ctx, nev, tol, max_cycles, filter_degree, block, phi_out):
+    """Returns (status, lambda[nev], residual[nev], cycles); phi_out is filled with nev canonical complex128 spinors."""
+    lam, res, cyc = (_D * nev)(), (_D * nev)(), _I(0)
+    rc = load_library().ovl_lowest_eigenpairs(ctx, int(nev), float(tol), int(max_cycles), int(filter_degree), int(block),
+                                              _ptr(phi_out), lam, res, C.byref(cyc))
+    _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, np.array(lam), np.array(res), int(cyc.value)
 
 
 def ovl_last_error(ctx) -> str:

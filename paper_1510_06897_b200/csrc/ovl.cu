@@ -1,6 +1,7 @@
 // ovl.cu -- the extern "C" entry points declared in include/ovl.h.  Argument checking, pointer staging
 // (host <-> device) and precision dispatch only; the arithmetic lives in ovl_wilson.cuh / ovl_blas.cuh.
 #include "ovl_engine.cuh"
+#include "ovl_eigsolve.cuh"
 
 using namespace ovl;
 
@@ -311,6 +312,16 @@ int ovl_cg_mixed(ovl_ctx *c, ovl_ctx *c32, double mu, const void *b, void *x, do
     if (rc2 != OVL_OK) return rc2;
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     return rc;
+}
+
+int ovl_lowest_eigenpairs(ovl_ctx *c, int nev, double tol, int max_cycles, int filter_degree, int block, void *phi_out,
+                          double *lambda_out, double *resid_out, int *cycles_out) {
+    if (!c) return OVL_EINVAL;
+    if (nev < 1 || !(tol > 0) || max_cycles < 0 || !phi_out || !lambda_out || !cycles_out || block < 0)
+        return fail(c, OVL_EINVAL, "bad ovl_lowest_eigenpairs arguments");
+    if (c->prec != OVL_F64) return fail(c, OVL_EINVAL, "the eigensolver needs an OVL_F64 context");
+    return eig_lowest(c, nev, tol, max_cycles, filter_degree > 0 ? filter_degree : 100, block, 1510068970ull, phi_out, lambda_out,
+                      resid_out, cycles_out);
 }
 
 const char *ovl_last_error(const ovl_ctx *c) { return c ? c->err : "null context"; }

@@ -1,0 +1,320 @@
+// ovl_eigsolve.cuh -- lowest-|lambda| eigenpairs of K = gamma5 (D_W - m_w) on the GPU.
+// (the paper: polynomial preconditioned implicitly restarted Lanczos).  K is indefinite, so a Rayleigh-Ritz step on K in a
+// not-yet-converged subspace produces ghost values inside the gap; the iteration therefore works on the positive K^2 and
+// K itself is diagonalised only at the end, inside a space that is K-invariant by construction:
+//
+//   V: m = nev + pad trial vectors.  Per cycle (Chebyshev-filtered block subspace iteration on K^2):
+//     W = K^ V                                   (multi-right-hand-side launches of the fused stencil kernel)
+//     G = V^dag V, H = W^dag W = V^dag K^2 V     (tall-skinny products, k_gram_block)
+//     H x = sigma G x on the host (Cholesky + Jacobi), ascending;  V <- V X, W <- W X            (k_rotate_block)
+//     Z = K^ W;  r_i = || Z_i - sigma_i V_i ||   (K^2 residuals)
+//     V <- T_d(Y) V,  Y = (K^2 - c)/e mapping [a, 1] -> [-1, 1],  a = largest sigma in the block (everything above the
+//          block is damped, the block is amplified);  T_{j+1} = 2 Y T_j - T_{j-1} costs two stencil launches per step
+//   End game, once the nev leading K^2 pairs have converged: for an eigenvector v of K^2, span{v, K v} is K-invariant
+//   (K (K v) = sigma v), so K is diagonalised in S = span{V_1..nev, W_1..nev}: orthonormal basis from the eigen-
+//   decomposition of S^dag S (directions below 1e-12 dropped), Hermitian eigenproblem of K in it, the nev Ritz pairs of
+//   smallest |theta| are returned (with their +-signs, R11) and their residuals recomputed with one more K^.
+#pragma once
+#include "ovl_dense.h"
+#include "ovl_eig.cuh"
+#include "ovl_engine.cuh"
+
+namespace ovl {
+
+struct EigWork {
+    double2 *V = nullptr, *W = nullptr, *Z = nullptr, *R = nullptr, *Q = nullptr, *gram_partial = nullptr, *C = nullptr, *X = nullptr;
+    double *partial = nullptr, *small = nullptr;  // small: theta / scales / norms, cap doubles each (3 cap)
+    int cap = 0;                                  // vectors per work block
+    ~EigWork() {
+        void *p[] = {V, W, Z, R, Q, gram_partial, C, X, partial, small};
+        for (void *q : p)
+            if (q) cudaFree(q);
+        cudaGetLastError();
+    }
+};
+
+// C (host, m x m row-major) = A^dag B for the m-vector blocks A, B
+inline int eig_gram(ovl_ctx *c, EigWork &w, int m, const double2 *A, const double2 *B, dense::mat &out) {
+    const size_t n = c->n();
+    const int nblk = (int)((n + BLAS_THREADS * GRAM_EPT - 1) / (BLAS_THREADS * GRAM_EPT));
+    const int nchunk = (m + GRAM_J - 1) / GRAM_J;
+    for (int ch = 0; ch < nchunk; ++ch) {
+        const int j0 = ch * GRAM_J, nj = std::min(GRAM_J, m - j0);
+        k_gram_block<<<nblk, BLAS_THREADS, 0, c->st>>>(n, m, nj, A, B + (size_t)j0 * n, w.gram_partial);
+        OVL_LAUNCH_CHECK(c);
+        k_gram_final<<<m * GRAM_J, BLAS_THREADS, 0, c->st>>>(nblk * (BLAS_THREADS / 32), w.gram_partial, w.C + (size_t)ch * m * GRAM_J);
+        OVL_LAUNCH_CHECK(c);
+    }
+    std::vector<double2> h((size_t)nchunk * m * GRAM_J);
+    OVL_CUDA(c, cudaMemcpyAsync(h.data(), w.C, h.size() * sizeof(double2), cudaMemcpyDeviceToHost, c->st));
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    out.assign((size_t)m * m, dense::cd(0, 0));
+    for (int ch = 0; ch < nchunk; ++ch)
+        for (int i = 0; i < m; ++i)
+            for (int jj = 0; jj < GRAM_J && ch * GRAM_J + jj < m; ++jj) {
+                const double2 v = h[((size_t)ch * m + i) * GRAM_J + jj];
+                out[(size_t)i * m + ch * GRAM_J + jj] = dense::cd(v.x, v.y);
+            }
+    return OVL_OK;
+}
+
+// dst block (nout vectors) = src block (nin vectors) * X  (X on the device, row-major nin x ldx, first nout columns)
+inline int eig_rotate(ovl_ctx *c, EigWork &w, int nin, int nout, int ldx, const double2 *src, double2 *dst) {
+    const size_t n = c->n();
+    for (int o0 = 0; o0 < nout; o0 += ROT_JO) {
+        const int no = std::min(ROT_JO, nout - o0);
+        k_rotate_block<<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(n, nin, no, ldx, w.X + o0, src, dst + (size_t)o0 * n);
+        OVL_LAUNCH_CHECK(c);
+    }
+    return OVL_OK;
+}
+
+// out_r = K^ in_r for a block of nvec consecutive native fields, OVL_MAX_RHS at a time
+inline int eig_khat_block(ovl_ctx *c, int nvec, const double2 *in, double2 *out) {
+    const size_t n = c->n();
+    for (int j0 = 0; j0 < nvec; j0 += OVL_MAX_RHS) {
+        WilsonArgs a;
+        a.nrhs = std::min((int)OVL_MAX_RHS, nvec - j0);
+        a.in = in + (size_t)j0 * n; a.out = out + (size_t)j0 * n;
+        a.c_diag = (4.0 - c->m_w) / c->lambda_max; a.c_hop = -0.5 / c->lambda_max;
+        OVL_TRY((launch_wilson<double, K_G5>(c, a)));
+    }
+    return OVL_OK;
+}
+
+// V_chunk <- T_d((K^2 - cc)/ee) V_chunk, with W_chunk = K^ V_chunk on entry (d >= 1)
+inline int eig_filter_chunk(ovl_ctx *c, int nv, int d, double cc, double ee, double2 *Vc, const double2 *Wc) {
+    const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
+    const size_t fb = c->field_bytes() * nv;
+    double2 *tcur = (double2 *)c->tA, *tprev = Vc, *wbuf = (double2 *)c->acc;
+    {   // t_1 = (K^ W - cc V)/ee
+        WilsonArgs a;
+        a.nrhs = nv; a.in = Wc; a.psi = Vc; a.out = tcur;
+        a.c_diag = cd / ee; a.c_hop = ch / ee; a.a_psi = -cc / ee;
+        OVL_TRY((launch_wilson<double, K_G5 | K_PSI>(c, a)));
+    }
+    for (int j = 1; j < d; ++j) {  // t_{j+1} = (2/ee) K^ (K^ t_j) - (2 cc/ee) t_j - t_{j-1}, written over t_{j-1}
+        WilsonArgs k;
+        k.nrhs = nv; k.in = tcur; k.out = wbuf; k.c_diag = cd; k.c_hop = ch;
+        OVL_TRY((launch_wilson<double, K_G5>(c, k)));
+        WilsonArgs a;
+        a.nrhs = nv; a.in = wbuf; a.psi = tcur; a.prev = tprev; a.out = tprev;
+        a.c_diag = 2.0 * cd / ee; a.c_hop = 2.0 * ch / ee; a.a_psi = -2.0 * cc / ee;
+        OVL_TRY((launch_wilson<double, K_G5 | K_PSI | K_PREV>(c, a)));
+        std::swap(tcur, tprev);
+    }
+    if (tcur != Vc) OVL_CUDA(c, cudaMemcpyAsync(Vc, tcur, fb, cudaMemcpyDeviceToDevice, c->st));
+    return OVL_OK;
+}
+
+// residual norms || A_i - theta_i B_i || for i < k into host vector (A, B blocks of k fields)
+inline int eig_resid(ovl_ctx *c, EigWork &w, int k, const std::vector<double> &theta, const double2 *A, const double2 *B, std::vector<double> &out) {
+    const int nb = c->red_nblk;
+    double *theta_d = w.small, *norm_d = w.small + 2 * w.cap;
+    OVL_CUDA(c, cudaMemcpyAsync(theta_d, theta.data(), sizeof(double) * k, cudaMemcpyHostToDevice, c->st));
+    k_resid_norm2<<<dim3(nb, k), BLAS_THREADS, 0, c->st>>>(c->n(), theta_d, A, B, w.partial);
+    OVL_LAUNCH_CHECK(c);
+    k_sum_partials<<<k, BLAS_THREADS, 0, c->st>>>(nb, w.partial, norm_d);
+    OVL_LAUNCH_CHECK(c);
+    out.resize(k);
+    OVL_CUDA(c, cudaMemcpyAsync(out.data(), norm_d, sizeof(double) * k, cudaMemcpyDeviceToHost, c->st));
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    for (double &x : out) x = std::sqrt(std::max(x, 0.0));
+    return OVL_OK;
+}
+
+// End game (see the header): K diagonalised in span{V_1..nev, W_1..nev}; the nev Ritz vectors of smallest |theta| are
+// written to w.Z[0..nev), theta (in units of lambda_max) and the true residuals || K^ z - theta z || to the outputs.
+inline int eig_endgame(ovl_ctx *c, EigWork &w, int nev, std::vector<double> &theta_out, std::vector<double> &resid_out) {
+    const size_t n = c->n(), fb = c->field_bytes();
+    const int k2 = 2 * nev;
+    // S = [V_1..nev, W_1..nev] in R, K S = [W_1..nev, Z_1..nev] in Q
+    OVL_CUDA(c, cudaMemcpyAsync(w.R, w.V, fb * nev, cudaMemcpyDeviceToDevice, c->st));
+    OVL_CUDA(c, cudaMemcpyAsync(w.R + (size_t)nev * n, w.W, fb * nev, cudaMemcpyDeviceToDevice, c->st));
+    OVL_CUDA(c, cudaMemcpyAsync(w.Q, w.W, fb * nev, cudaMemcpyDeviceToDevice, c->st));
+    OVL_CUDA(c, cudaMemcpyAsync(w.Q + (size_t)nev * n, w.Z, fb * nev, cudaMemcpyDeviceToDevice, c->st));
+    dense::mat G, H, Qm, Y;
+    OVL_TRY(eig_gram(c, w, k2, w.R, w.R, G));
+    OVL_TRY(eig_gram(c, w, k2, w.R, w.Q, H));
+    std::vector<double> lamG, th;
+    dense::mat Gc = G;
+    dense::jacobi_eigh(Gc, k2, lamG, Qm);
+    double gmax = 0;
+    for (double x : lamG) gmax = std::max(gmax, x);
+    std::vector<int> keep;
+    for (int i = 0; i < k2; ++i)
+        if (lamG[i] > 1e-12 * gmax) keep.push_back(i);
+    const int r = (int)keep.size();
+    if (r < nev) return fail(c, OVL_ECUDA, "eigensolver: end-game space has dimension %d < nev", r);
+    // T = Q_keep Lambda^{-1/2}  (k2 x r);  Hr = T^dag H T
+    dense::mat T((size_t)k2 * r), HT((size_t)k2 * r), Hr((size_t)r * r);
+    for (int i = 0; i < k2; ++i)
+        for (int a = 0; a < r; ++a) T[(size_t)i * r + a] = Qm[(size_t)i * k2 + keep[a]] / std::sqrt(lamG[keep[a]]);
+    for (int i = 0; i < k2; ++i)
+        for (int a = 0; a < r; ++a) {
+            dense::cd s = 0;
+            for (int j = 0; j < k2; ++j) s += 0.5 * (H[(size_t)i * k2 + j] + std::conj(H[(size_t)j * k2 + i])) * T[(size_t)j * r + a];
+            HT[(size_t)i * r + a] = s;
+        }
+    for (int a = 0; a < r; ++a)
+        for (int b = 0; b < r; ++b) {
+            dense::cd s = 0;
+            for (int i = 0; i < k2; ++i) s += std::conj(T[(size_t)i * r + a]) * HT[(size_t)i * r + b];
+            Hr[(size_t)a * r + b] = s;
+        }
+    for (int a = 0; a < r; ++a)
+        for (int b = a; b < r; ++b) {
+            const dense::cd v = 0.5 * (Hr[(size_t)a * r + b] + std::conj(Hr[(size_t)b * r + a]));
+            Hr[(size_t)a * r + b] = v;
+            Hr[(size_t)b * r + a] = std::conj(v);
+        }
+    dense::jacobi_eigh(Hr, r, th, Y);
+    std::vector<int> order(r);
+    for (int i = 0; i < r; ++i) order[i] = i;
+    std::sort(order.begin(), order.end(), [&](int a, int b) { return std::fabs(th[a]) < std::fabs(th[b]); });
+    // coefficients of the nev chosen Ritz vectors in S: X = T Y[:, order[:nev]]   (k2 x nev)
+    std::vector<double2> xs((size_t)k2 * nev);
+    theta_out.resize(nev);
+    for (int o = 0; o < nev; ++o) {
+        theta_out[o] = th[order[o]];
+        for (int i = 0; i < k2; ++i) {
+            dense::cd s = 0;
+            for (int a = 0; a < r; ++a) s += T[(size_t)i * r + a] * Y[(size_t)a * r + order[o]];
+            xs[(size_t)i * nev + o] = make_double2(s.real(), s.imag());
+        }
+    }
+    OVL_CUDA(c, cudaMemcpyAsync(w.X, xs.data(), xs.size() * sizeof(double2), cudaMemcpyHostToDevice, c->st));
+    OVL_TRY(eig_rotate(c, w, k2, nev, nev, w.R, w.Z));
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));  // xs is pageable host memory
+    OVL_TRY(eig_khat_block(c, nev, w.Z, w.Q));
+    return eig_resid(c, w, nev, theta_out, w.Q, w.Z, resid_out);
+}
+
+inline int eig_lowest(ovl_ctx *c, int nev, double tol, int max_cycles, int degree, int block, unsigned long long seed,
+                      void *phi_out, double *lambda_out, double *resid_out, int *cycles_out) {
+    const size_t n = c->n();
+    int m = block > 0 ? block : nev + std::max(8, nev / 2);
+    if (m < nev) m = nev;
+    if (m > 128 || nev > 64) return fail(c, OVL_EINVAL, "block size %d > 128 or nev %d > 64", m, nev);
+    if ((size_t)m > n) return fail(c, OVL_EINVAL, "block size %d exceeds the dimension of the space", m);
+    if (degree < 1) degree = 1;
+    const int cap = std::max(m, 2 * nev);  // vectors per work block
+    const int chunk = std::min(m, (int)OVL_MAX_RHS);
+    OVL_TRY(ensure_work(c, chunk));
+    EigWork w;
+    w.cap = cap;
+    const size_t bb = c->field_bytes() * cap;
+    const int nblk_g = (int)((n + BLAS_THREADS * GRAM_EPT - 1) / (BLAS_THREADS * GRAM_EPT));
+    const int nchunk_g = (cap + GRAM_J - 1) / GRAM_J;
+    const int nb = c->red_nblk;
+    OVL_CUDA(c, cudaMalloc((void **)&w.V, bb));
+    OVL_CUDA(c, cudaMalloc((void **)&w.W, bb));
+    OVL_CUDA(c, cudaMalloc((void **)&w.Z, bb));
+    OVL_CUDA(c, cudaMalloc((void **)&w.R, bb));
+    OVL_CUDA(c, cudaMalloc((void **)&w.Q, c->field_bytes() * 2 * nev));
+    OVL_CUDA(c, cudaMalloc((void **)&w.gram_partial, sizeof(double2) * (size_t)cap * GRAM_J * nblk_g * (BLAS_THREADS / 32)));
+    OVL_CUDA(c, cudaMalloc((void **)&w.C, sizeof(double2) * (size_t)nchunk_g * cap * GRAM_J));
+    OVL_CUDA(c, cudaMalloc((void **)&w.X, sizeof(double2) * (size_t)cap * cap));
+    OVL_CUDA(c, cudaMalloc((void **)&w.partial, sizeof(double) * (size_t)nb * cap));
+    OVL_CUDA(c, cudaMalloc((void **)&w.small, sizeof(double) * 3 * cap));
+    double *scale_d = w.small + cap, *norm_d = w.small + 2 * cap;
+
+    for (int j = 0; j < m; ++j) {
+        k_fill_random<<<grid_for(n, BLAS_THREADS), BLAS_THREADS, 0, c->st>>>(n, seed * 1000003ull + j, w.V + (size_t)j * n);
+        OVL_LAUNCH_CHECK(c);
+    }
+    std::vector<double> sigma(m), r2, hs(m), theta, resid;
+    std::vector<int> order(m);
+    dense::mat G, H, X;
+    int cycle = 0;
+    bool converged = false, have_result = false;
+    double tol_int = 0.5 * tol / c->lambda_max;  // on || K^ z - theta z ||; tightened if the end game misses tol
+    for (;;) {
+        OVL_TRY(eig_khat_block(c, m, w.V, w.W));
+        OVL_TRY(eig_gram(c, w, m, w.V, w.V, G));
+        OVL_TRY(eig_gram(c, w, m, w.W, w.W, H));
+        std::vector<double> sg;
+        if (!dense::geneig(H, G, m, sg, X))
+            return fail(c, OVL_ECUDA, "eigensolver: the trial block became linearly dependent (cycle %d)", cycle);
+        for (int i = 0; i < m; ++i) order[i] = i;
+        std::sort(order.begin(), order.end(), [&](int a, int b) { return sg[a] < sg[b]; });
+        std::vector<double2> xs((size_t)m * m);
+        for (int j = 0; j < m; ++j)
+            for (int o = 0; o < m; ++o) {
+                const dense::cd v = X[(size_t)j * m + order[o]];
+                xs[(size_t)j * m + o] = make_double2(v.real(), v.imag());
+            }
+        for (int o = 0; o < m; ++o) sigma[o] = std::max(sg[order[o]], 0.0);
+        OVL_CUDA(c, cudaMemcpyAsync(w.X, xs.data(), xs.size() * sizeof(double2), cudaMemcpyHostToDevice, c->st));
+        OVL_TRY(eig_rotate(c, w, m, m, m, w.V, w.R));
+        std::swap(w.V, w.R);
+        OVL_TRY(eig_rotate(c, w, m, m, m, w.W, w.R));
+        std::swap(w.W, w.R);
+        OVL_CUDA(c, cudaStreamSynchronize(c->st));  // xs is pageable host memory
+        OVL_TRY(eig_khat_block(c, m, w.W, w.Z));
+        OVL_TRY(eig_resid(c, w, m, sigma, w.Z, w.V, r2));
+        // K^2 residual r2 <-> K residual r2 / |theta| of the vectors v +- K v / theta
+        double worst = 0;
+        for (int i = 0; i < nev; ++i) worst = std::max(worst, r2[i] / std::max(std::sqrt(sigma[i]), 1e-300));
+        if (worst <= tol_int) {
+            OVL_TRY(eig_endgame(c, w, nev, theta, resid));
+            have_result = true;
+            double wr = 0;
+            for (int i = 0; i < nev; ++i) wr = std::max(wr, resid[i] * c->lambda_max);
+            if (wr <= tol) { converged = true; break; }
+            tol_int *= 0.1;
+        }
+        if (cycle >= max_cycles) break;
+        ++cycle;
+        // filter: damp [a, 1] of K^2, a = top of the block
+        const double a = std::min(sigma[m - 1], 0.95);
+        const double cc = 0.5 * (1.0 + a), ee = 0.5 * (1.0 - a);
+        for (int j0 = 0; j0 < m; j0 += chunk) {
+            const int nv = std::min(chunk, m - j0);
+            OVL_TRY(eig_filter_chunk(c, nv, degree, cc, ee, w.V + (size_t)j0 * n, w.W + (size_t)j0 * n));
+        }
+        // normalise
+        k_redot<double><<<dim3(nb, m), BLAS_THREADS, 0, c->st>>>(n, w.V, w.V, w.partial);
+        OVL_LAUNCH_CHECK(c);
+        k_sum_partials<<<m, BLAS_THREADS, 0, c->st>>>(nb, w.partial, norm_d);
+        OVL_LAUNCH_CHECK(c);
+        OVL_CUDA(c, cudaMemcpyAsync(hs.data(), norm_d, sizeof(double) * m, cudaMemcpyDeviceToHost, c->st));
+        OVL_CUDA(c, cudaStreamSynchronize(c->st));
+        for (int i = 0; i < m; ++i) {
+            if (!(hs[i] > 0) || !std::isfinite(hs[i])) return fail(c, OVL_ECUDA, "eigensolver: filtered vector %d has norm^2 %g", i, hs[i]);
+            hs[i] = 1.0 / std::sqrt(hs[i]);
+        }
+        OVL_CUDA(c, cudaMemcpyAsync(scale_d, hs.data(), sizeof(double) * m, cudaMemcpyHostToDevice, c->st));
+        k_scale_batched<<<dim3(grid_for(n, BLAS_THREADS), m), BLAS_THREADS, 0, c->st>>>(n, scale_d, w.V);
+        OVL_LAUNCH_CHECK(c);
+        OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    }
+    if (!have_result) OVL_TRY(eig_endgame(c, w, nev, theta, resid));  // best effort on the unconverged block
+    // results: nev Ritz pairs of K in w.Z
+    const size_t cb = n * sizeof(double2);
+    for (int i = 0; i < nev; ++i) {
+        lambda_out[i] = theta[i] * c->lambda_max;
+        if (resid_out) resid_out[i] = resid[i] * c->lambda_max;
+        void *dst = (char *)phi_out + (size_t)i * cb;
+        if (is_device_ptr(phi_out)) {
+            k_export_spinor<double, double><<<grid_for(n, BLAS_THREADS), BLAS_THREADS, 0, c->st>>>(c->g.V, w.Z + (size_t)i * n, (double2 *)dst);
+            OVL_LAUNCH_CHECK(c);
+        } else {
+            OVL_TRY(dev_alloc(c, &c->stage_out, cb));
+            k_export_spinor<double, double><<<grid_for(n, BLAS_THREADS), BLAS_THREADS, 0, c->st>>>(c->g.V, w.Z + (size_t)i * n, (double2 *)c->stage_out);
+            OVL_LAUNCH_CHECK(c);
+            OVL_CUDA(c, cudaMemcpyAsync(dst, c->stage_out, cb, cudaMemcpyDeviceToHost, c->st));
+            OVL_CUDA(c, cudaStreamSynchronize(c->st));
+        }
+    }
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    *cycles_out = cycle;
+    if (!converged) {
+        double worst = 0;
+        for (int i = 0; i < nev; ++i) worst = std::max(worst, resid[i] * c->lambda_max);
+        return fail(c, OVL_ENOTCONV, "eigensolver: %d cycles, largest residual ||K phi - lambda phi|| = %.3e > tol", cycle, worst);
+    }
+    return OVL_OK;
+}
+
+}  // namespace ovl

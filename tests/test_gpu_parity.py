@@ -431,6 +431,73 @@ def test_cg_mixed_precision(torch, api, orc):
                 B.ovl_cg_mixed(op.ctx, other.ctx, mu, bd, out, 1e-8, 1e-4, 5, 100)
 
 
+def test_eigensolver_4x4_against_dense_spectrum(torch, api, orc, dense44):
+    """ovl_lowest_eigenpairs on the config-0 lattice: eigenvalues against the dense spectrum of the
+    oracle's K (both signs), residuals recomputed with the ORACLE's K, orthonormality, and the pairs used as a
+    deflation space: sign(K) phi_i = sign(lambda_i) phi_i even with a poor polynomial."""
+    d = dense44
+    dims, U = d["dims"], d["U"]
+    nev = 12
+    ev = d["lam"][np.argsort(np.abs(d["lam"]))][:nev]
+    with api.Overlap(dims, dev(torch, U)) as op:
+        phi, lam, res, cyc, ok = op.lowest_eigenpairs(nev, tol=1e-9, filter_degree=40)
+        assert ok and cyc > 0 and res.max() <= 1e-9
+        assert np.abs(np.sort(lam) - np.sort(ev)).max() < 1e-10
+        assert (lam > 0).any() and (lam < 0).any()
+        ph = host(phi)
+        gram = np.einsum("ixsc,jxsc->ij", ph.conj(), ph)
+        assert np.abs(gram - np.eye(nev)).max() < 1e-10
+        for i in (0, 5, nev - 1):
+            r = orc.khat(dims, U, ph[i], 1.5, 6.5) * 6.5 - lam[i] * ph[i]
+            assert np.linalg.norm(r) < 5e-9 and abs(np.linalg.norm(r) - res[i]) < 1e-9
+        op.set_chebyshev(inputs.chebyshev_sign_coeffs(11, 0.3))
+        op.set_deflation(phi, lam)
+        for i in (0, nev - 1):
+            s = host(op.sign(phi[i].contiguous()))
+            assert rel_err(s, np.sign(lam[i]) * ph[i]) < 1e-8
+
+
+def test_eigensolver_config1_lattice(torch, api, orc):
+    """The deflation space of BASELINE config 1 computed on the GPU: 8^3 x 32, 20 pairs.  (i) pure gauge: |lambda| equals
+    the closed-form lowest level (24-fold, tests/closed_forms.py); (ii) the smeared config-1 links: residuals checked
+    with the oracle's K, both signs present, nearly degenerate +-pairs resolved."""
+    from tests.closed_forms import free_sign_fft, golden_gammas
+    dims, nev = (8, 8, 8, 32), 20
+    U, g = inputs.pure_gauge_links(dims, inputs.SEED_BASE + 31)
+    _, omega = free_sign_fft(dims, inputs.gaussian_spinor(dims, 1), golden_gammas(), 1.5, g)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        phi, lam, res, cyc, ok = op.lowest_eigenpairs(nev, tol=1e-8, filter_degree=200, block=40)
+    assert ok and np.abs(np.abs(lam) - omega.min()).max() < 1e-9
+    U = inputs.config_links(dims, 0.3, inputs.SEED_BASE + 1, stout_steps=3)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        phi, lam, res, cyc, ok = op.lowest_eigenpairs(nev, tol=1e-8, filter_degree=200, block=40)
+        ph = host(phi)
+    assert ok and res.max() <= 1e-8 and (lam > 0).any() and (lam < 0).any()
+    assert 0.45 < np.abs(lam).min() and np.abs(lam).max() < 0.56 and np.all(np.diff(np.abs(lam)) >= -1e-12)
+    for i in (0, 9, 19):
+        r = orc.khat(dims, U, ph[i], 1.5, 6.5) * 6.5 - lam[i] * ph[i]
+        assert np.linalg.norm(r) < 5e-8
+    gram = np.einsum("ixsc,jxsc->ij", ph.conj(), ph)
+    assert np.abs(gram - np.eye(nev)).max() < 1e-9
+
+
+def test_eigensolver_argument_checks(torch, api):
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 4, 4)
+    U = inputs.random_links(dims, 0.3, 3)
+    with api.Overlap(dims, U, "f32") as op32:
+        phi = torch.empty((2, 256, 4, 3), dtype=torch.complex128, device="cuda")
+        with pytest.raises(B.OvlError) as e:
+            B.ovl_lowest_eigenpairs(op32.ctx, 2, 1e-6, 5, 20, 0, phi)
+        assert e.value.code == B.OVL_EINVAL
+    with api.Overlap(dims, U) as op:
+        phi, lam, res, cyc, ok = op.lowest_eigenpairs(4, tol=1e-14, max_cycles=1, filter_degree=5)
+        assert not ok and cyc == 1 and np.isfinite(lam).all()      # OVL_ENOTCONV, best Ritz pairs returned
+        out = np.empty((3, 256, 4, 3), dtype=np.complex128)         # host output buffer
+        rc, lam, res, cyc = B.ovl_lowest_eigenpairs(op.ctx, 3, 1e-8, 60, 40, 0, out)
+        assert rc == B.OVL_OK and abs(np.vdot(out[0], out[0]) - 1) < 1e-10
+
+
 def test_multi_rhs_host_pointers_and_errors(torch, api, orc):
     from paper_1510_06897_b200 import binding as B
     dims = (4, 4, 4, 6)
