@@ -486,6 +486,8 @@ def run_native(args, w):
                                         "orders": r1["orders"]}
             extras["cfg2_cg"] = bench_cg(torch, api, w1)
             extras["cfg1_eigensolver"] = bench_eigensolver(torch, api, w1, 20, 40, 200)
+            if args.cfg3_eigensolver:  # ~40 s: the 50 pairs of config 3 (block 104 reaches past the 24 + 72 clusters)
+                extras["cfg3_eigensolver"] = bench_eigensolver(torch, api, w, 50, 104, 200)
             extras["cfg2_cg_12rhs"] = bench_cg_multi(torch, api, w1)
             extras["cfg2_cg_mixed"] = bench_cg_mixed(torch, api, w1, label="config 2 (8^3x32, mu=0.05, tol 1e-8)")
             extras["cfg3_cg_mixed"] = bench_cg_mixed(torch, api, w, host_inputs,
@@ -527,6 +529,8 @@ def main():
                     help="evaluation order of the polynomial sum of eq. 2.3 (ovl_set_recurrence)")
     ap.add_argument("--ref-orders", type=int, default=12, help="polynomial orders in the oracle's bounded sample")
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--cfg3-eigensolver", action="store_true",
+                    help="extras: also compute the 50 deflation pairs of config 3 on the GPU (ovl_lowest_eigenpairs, ~40 s)")
     ap.add_argument("--fast-inputs", action="store_true",
                     help="profiling runs only: skip the stout smearing of the links (same shapes, same kernels, same "
                          "bytes; the config string says so)")
