@@ -105,7 +105,7 @@ class ClockSampler:
     """Samples SM clock and throttle reasons during the timed region (NVML; nvidia-smi fallback)."""
 
     def __init__(self, index=0, period=0.02):
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.reasons, self.max_mhz, self.power, self.mem = [], set(), None, [], []
         self._stop = threading.Event()
         self._thr = None
         self.index, self.period = index, period
@@ -126,6 +126,11 @@ class ClockSampler:
         while not self._stop.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                    self.mem.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_MEM))
+                except Exception:
+                    pass
                 try:
                     r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
                 except Exception:
@@ -150,7 +155,10 @@ class ClockSampler:
         if self.nv is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
         med = float(np.median(self.samples)) if self.samples else None
-        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "sm_mhz_min": float(min(self.samples)) if self.samples else None,
+                "power_w": float(np.median(self.power)) if self.power else None,
+                "mem_mhz": float(np.median(self.mem)) if self.mem else None}
 
 
 def measured_peaks():
@@ -500,6 +508,11 @@ def run_native(args, w):
                                     args.recurrence)
                 extras["cfg3_fp32"] = {"applies_per_s": r32["applies_per_s"], "achieved_gbs": r32["achieved_gbs"],
                                        "frac": r32["achieved_gbs"] / hbm_peak, "kernel_us": r32["kernel_us"]}
+            if args.recon == 18:
+                r12 = bench_overlap(torch, api, B, w, args.prec, 12, args.steps, args.warmup, None, 0, False, host_inputs, args.recurrence)
+                extras["cfg3_12real_links"] = {"applies_per_s": r12["applies_per_s"], "achieved_gbs": r12["achieved_gbs"],
+                                               "frac": r12["achieved_gbs"] / hbm_peak, "kernel_us": r12["kernel_us"],
+                                               "algorithmic_bytes_per_site_per_launch": r12["bytes_per_site_per_order"]}
             other = "forward" if args.recurrence == "clenshaw" else "clenshaw"
             ro = bench_overlap(torch, api, B, w, args.prec, args.recon, args.steps, args.warmup, None, 0, False, host_inputs, other)
             extras[f"cfg3_{other}_recurrence"] = {
