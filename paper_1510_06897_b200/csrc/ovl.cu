@@ -15,7 +15,7 @@ int check_cfg(const int dims[4], int prec, int recon) {
     for (int i = 0; i < 4; ++i) {
         if (dims[i] < 2) return OVL_EINVAL;
         v *= dims[i];
-        if (v > (1ll << 27)) return OVL_EINVAL;  // plane stride V * 16 B is kept in 32 bits (ovl_types.cuh: plane())
+        if (v > (1ll << 30)) return OVL_EINVAL;
     }
     if (prec != OVL_F64 && prec != OVL_F32) return OVL_EINVAL;
     if (recon != OVL_RECON18 && recon != OVL_RECON12) return OVL_EINVAL;

@@ -51,15 +51,4 @@ struct Geom {
 __device__ __forceinline__ double2 ldg(const double2 *p) { return __ldg(p); }
 __device__ __forceinline__ float2 ldg(const float2 *p) { return __ldg(p); }
 
-// Address of plane k of a field for one site: base = &field[site] (one 64-bit address per site), planes are psb =
-// V * sizeof(complex) bytes apart.  Written as base + k * psb with a 32-bit psb so that every plane address is ONE
-// IMAD.WIDE.U32 (k is a compile-time constant after unrolling) instead of a 64-bit multiply-shift-add chain: the
-// fused kernel issues ~200 loads per site and a third of its instructions were address arithmetic.
-template <typename C> __device__ __forceinline__ const C *plane(const C *base, int k, unsigned psb) {
-    return reinterpret_cast<const C *>(reinterpret_cast<const char *>(base) + (unsigned long long)((unsigned)k) * psb);
-}
-template <typename C> __device__ __forceinline__ C *plane(C *base, int k, unsigned psb) {
-    return reinterpret_cast<C *>(reinterpret_cast<char *>(base) + (unsigned long long)((unsigned)k) * psb);
-}
-
 }  // namespace ovl

@@ -53,7 +53,7 @@ __device__ __forceinline__ void load_link(cx<T> (&u)[3][3], const cx<T> *__restr
 #pragma unroll
     for (int r = 0; r < NROW; ++r)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) u[r][c] = ldg(plane(Umu + su, r * 3 + c, (unsigned)V * (unsigned)sizeof(cx<T>)));
+        for (int c = 0; c < 3; ++c) u[r][c] = ldg(Umu + (size_t)(r * 3 + c) * V + su);
     if (RECON == 12) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -74,7 +74,7 @@ __device__ __forceinline__ void hop_dir(cx<T> (&hop)[12], const cx<T> *__restric
     constexpr int NROW = RECON == 18 ? 3 : 2;
     cx<T> p[12];
 #pragma unroll
-    for (int k = 0; k < 12; ++k) p[k] = ldg(plane(in + sn, k, (unsigned)V * (unsigned)sizeof(cx<T>)));
+    for (int k = 0; k < 12; ++k) p[k] = ldg(in + (size_t)k * V + sn);
     cx<T> u[3][3];
     load_link<T, RECON>(u, U + (size_t)MU * NROW * 3 * V, V, su);
 
@@ -174,20 +174,20 @@ k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restric
     const int y = (s / g.L[0]) % g.L[1];
     const int z = (s / g.sxy) % g.L[2];
     const int t = s / g.sxyz;
-    const unsigned psb = (unsigned)g.V * (unsigned)sizeof(cx<T>);  // bytes between planes (V <= 2^27 checked at create)
+    const size_t V = g.V;
 
     // accumulators start from the site-local terms (no loads are left for the epilogue)
     cx<T> hop[12];
 #pragma unroll
     for (int k = 0; k < 12; ++k) {
-        const cx<T> c = ldg(plane(in + s, k, psb));
+        const cx<T> c = ldg(in + k * V + s);
         hop[k].x = sp.r_c * c.x;
         hop[k].y = sp.r_c * c.y;
     }
     if (FLAGS & K_PREV) {
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const cx<T> pv = ldg(plane(prev + s, k, psb));
+            const cx<T> pv = ldg(prev + k * V + s);
             const T r = ((FLAGS & K_G5) && k >= 6) ? sp.r_p : -sp.r_p;
             hop[k].x = fma(r, pv.x, hop[k].x);
             hop[k].y = fma(r, pv.y, hop[k].y);
@@ -196,7 +196,7 @@ k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restric
     if (FLAGS & K_PSI) {
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const cx<T> ps = ldg(plane(psi + s, k, psb));
+            const cx<T> ps = ldg(psi + k * V + s);
             const T r = ((FLAGS & K_G5) && k >= 6) ? -sp.r_a : sp.r_a;
             hop[k].x = fma(r, ps.x, hop[k].x);
             hop[k].y = fma(r, ps.y, hop[k].y);
@@ -214,19 +214,19 @@ k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restric
         cx<T> w;
         w.x = f * hop[k].x;
         w.y = f * hop[k].y;
-        if (!(FLAGS & K_NOWRITE)) *plane(out + s, k, psb) = w;
+        if (!(FLAGS & K_NOWRITE)) out[k * V + s] = w;
         if (FLAGS & K_ACCI) {
-            const cx<T> c = ldg(plane(in + s, k, psb));
+            const cx<T> c = ldg(in + k * V + s);
             cx<T> a;
             a.x = fma(sp.a_init, c.x, sp.a_acc * w.x);
             a.y = fma(sp.a_init, c.y, sp.a_acc * w.y);
-            *plane(acc + s, k, psb) = a;
+            acc[k * V + s] = a;
         }
         if (FLAGS & K_ACC) {
-            cx<T> a = *plane(acc + s, k, psb);
+            cx<T> a = acc[k * V + s];
             a.x = fma(sp.a_acc, w.x, a.x);
             a.y = fma(sp.a_acc, w.y, a.y);
-            *plane(acc + s, k, psb) = a;
+            acc[k * V + s] = a;
         }
     }
 }
