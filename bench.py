@@ -40,10 +40,10 @@ WORKLOADS = {
                  desc="4^3x8 smoke-sized workload (not a benchmark)"),
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full` capture
-# (profiles/r1b_full.md: 681.0 MB with the psi term, 594.2 MB without, 198 : 199 launches per apply) -- bench.py cannot
+# (profiles/r1c_full.md: 682.1 MB with the psi term, 596.3 MB without, 198 : 199 launches per apply) -- bench.py cannot
 # run ncu itself; the value is reported only for the exact configuration that capture was taken on.
-NCU_TRAFFIC = {("cfg3", "f64", 18, "clenshaw"): {"bytes_per_launch": (198 * 681.1e6 + 199 * 594.2e6) / 397,
-                                                 "source": "profiles/r1b_full.md"}}
+NCU_TRAFFIC = {("cfg3", "f64", 18, "clenshaw"): {"bytes_per_launch": (198 * 682.1e6 + 199 * 596.3e6) / 397,
+                                                 "source": "profiles/r1c_full.md"}}
 METRIC = "overlap D[mu]psi applies/s"
 UNIT = "applies/s"
 

@@ -30,10 +30,14 @@ struct WilsonArgs {
 template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx *c, const WilsonArgs &a) {
     constexpr int TH = WilsonCfg<T>::THREADS;
     const int grid = ((c->g.V + TH - 1) / TH) * a.nrhs;
-    StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip,
-                     a.nrhs, c->n()};
-    k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
-        c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp);
+    StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip};
+    if (a.nrhs > 1)
+        k_wilson_fused_multi<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
+            c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp,
+            a.nrhs, c->n());
+    else
+        k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
+            c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp);
 }
 
 template <typename T, int FLAGS> inline int launch_wilson(ovl_ctx *c, const WilsonArgs &a) {

@@ -42,10 +42,7 @@ enum : int { K_G5 = 1, K_PREV = 2, K_PSI = 4, K_ACC = 8, K_ACCI = 16, K_NOWRITE 
 template <typename T> struct StepParams {
     T c_hop, r_c, r_p, r_a, a_acc, a_init;
     int flip;
-    int nrhs;        // right-hand sides processed by this launch; field r starts at r * fstride
-    size_t fstride;  // complex elements between consecutive right-hand sides (12 V)
 };
-
 // Load the 3x3 link U_mu(su) (rows r, cols c) from the native planes; rebuild row 2 for 12-real storage.
 template <typename T, int RECON>
 __device__ __forceinline__ void load_link(cx<T> (&u)[3][3], const cx<T> *__restrict__ Umu, int V, int su) {
@@ -147,29 +144,13 @@ __device__ __forceinline__ void hop_pair(cx<T> (&hop)[12], const cx<T> *__restri
     hop_dir<T, RECON, MU, 0>(hop, in, U, g.V, sb, sb, bb);
 }
 
-template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB)
-k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *__restrict__ prev,
-               const cx<T> *__restrict__ psi, cx<T> *__restrict__ out, cx<T> *__restrict__ acc, const StepParams<T> sp) {
-    // blockIdx.x = rhs + nrhs * tile: the CTAs that work on the same tile for different right-hand sides are adjacent in
-    // launch order, so they run at the same time and the tile's links come from DRAM once and from L2 after that
-    int rhs = 0, ntile = gridDim.x, tile = blockIdx.x;
-    if (sp.nrhs > 1) {
-        rhs = blockIdx.x % sp.nrhs;
-        ntile = gridDim.x / sp.nrhs;
-        tile = blockIdx.x / sp.nrhs;
-    }
-    if (sp.flip) tile = ntile - 1 - tile;
+// The kernel body for one tile of THREADS consecutive sites of one right-hand side.
+template <typename T, int RECON, int FLAGS, int THREADS>
+__device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in,
+                                            const cx<T> *__restrict__ prev, const cx<T> *__restrict__ psi, cx<T> *__restrict__ out,
+                                            cx<T> *__restrict__ acc, const StepParams<T> &sp, int tile) {
     const int s = tile * THREADS + threadIdx.x;
     if (s >= g.V) return;
-    {
-        const size_t off = (size_t)rhs * sp.fstride;
-        in += off;
-        if (FLAGS & K_PREV) prev += off;
-        if (FLAGS & K_PSI) psi += off;
-        if (!(FLAGS & K_NOWRITE)) out += off;
-        if (FLAGS & (K_ACC | K_ACCI)) acc += off;
-    }
     const int x = s % g.L[0];
     const int y = (s / g.L[0]) % g.L[1];
     const int z = (s / g.sxy) % g.L[2];
@@ -229,6 +210,29 @@ k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restric
             acc[k * V + s] = a;
         }
     }
+}
+
+// Single right-hand side: the field pointers stay kernel parameters (constant bank).
+template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *__restrict__ prev,
+               const cx<T> *__restrict__ psi, cx<T> *__restrict__ out, cx<T> *__restrict__ acc, const StepParams<T> sp) {
+    const int tile = sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    wilson_tile<T, RECON, FLAGS, THREADS>(g, U, in, prev, psi, out, acc, sp, tile);
+}
+
+// Several right-hand sides: blockIdx.x = rhs + nrhs * tile, so the CTAs that work on the same
+// tile for different right-hand sides are adjacent in launch order, run at the same time, and the tile's links come from
+// DRAM once and from L2 after that.  Field r starts r * fstride complex elements after field 0.
+template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_wilson_fused_multi(const Geom g, const cx<T> *__restrict__ U, const cx<T> *in, const cx<T> *prev, const cx<T> *psi, cx<T> *out,
+                     cx<T> *acc, const StepParams<T> sp, int nrhs, size_t fstride) {
+    const int ntile = gridDim.x / nrhs, btile = blockIdx.x / nrhs;
+    const int tile = sp.flip ? ntile - 1 - btile : btile;
+    const size_t off = (size_t)(blockIdx.x % nrhs) * fstride;
+    wilson_tile<T, RECON, FLAGS, THREADS>(g, U, in + off, (FLAGS & K_PREV) ? prev + off : prev, (FLAGS & K_PSI) ? psi + off : psi,
+                                          (FLAGS & K_NOWRITE) ? out : out + off, (FLAGS & (K_ACC | K_ACCI)) ? acc + off : acc, sp, tile);
 }
 
 }  // namespace ovl
