@@ -60,7 +60,10 @@ enum { OVL_REC_CLENSHAW = 0, OVL_REC_FORWARD = 1 }; /* how sum_m alpha_m T_m(K^)
 /* Library version string, e.g. "ovl-b200 0.1 (sm_100a)". */
 const char *ovl_version(void);
 
-/* Device bytes a context for this configuration allocates (links + work vectors + max_nev eigenvectors). */
+/* Device bytes a context for this configuration allocates (links + work vectors + max_nev eigenvectors) when it is used
+ * with one right-hand side at a time.  On top of that: ovl_overlap_multi / ovl_cg_multi grow the recurrence and CG
+ * workspaces to nrhs fields each (8 * (nrhs - 1) more fields, kept until ovl_destroy), ovl_cg allocates its 4 vectors on
+ * first use, and ovl_lowest_eigenpairs needs 4 * max(block, 2 nev) + 2 nev fields while it runs. */
 size_t ovl_device_bytes(const int dims[4], int prec, int recon, int max_nev);
 
 /* Create a context: re-lay-out the links (S2; SoA site-coalesced planes, optional 12-real compression) and
