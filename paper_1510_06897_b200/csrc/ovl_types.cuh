@@ -51,4 +51,12 @@ struct Geom {
 __device__ __forceinline__ double2 ldg(const double2 *p) { return __ldg(p); }
 __device__ __forceinline__ float2 ldg(const float2 *p) { return __ldg(p); }
 
+// 16- or 8-byte asynchronous global -> shared copy of one complex (LDGSTS), and its completion wait
+template <typename C> __device__ __forceinline__ void cp_async_cx(C *smem, const C *gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    if (sizeof(C) == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 }  // namespace ovl

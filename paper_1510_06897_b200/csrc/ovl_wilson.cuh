@@ -144,6 +144,19 @@ __device__ __forceinline__ void hop_pair(cx<T> (&hop)[12], const cx<T> *__restri
     hop_dir<T, RECON, MU, 0>(hop, in, U, g.V, sb, sb, bb);
 }
 
+// Forward recurrence only: landing buffer of the accumulator stream.  acc(x) is needed after the whole stencil; loading it
+// there exposes a DRAM round trip per thread, loading it into registers at the top costs 48 registers.  It is copied
+// global -> shared with cp.async at the top instead (each thread its own 12 elements, so no barrier) and read back in the
+// epilogue: 24 KB per CTA in fp64.
+template <typename T, int THREADS, bool ENABLE> __device__ __forceinline__ cx<T> *acc_stage() {
+    if constexpr (ENABLE) {
+        __shared__ cx<T> buf[12 * THREADS];
+        return buf;
+    } else {
+        return nullptr;
+    }
+}
+
 // The kernel body for one tile of THREADS consecutive sites of one right-hand side.
 template <typename T, int RECON, int FLAGS, int THREADS>
 __device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in,
@@ -156,6 +169,12 @@ __device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restri
     const int z = (s / g.sxy) % g.L[2];
     const int t = s / g.sxyz;
     const size_t V = g.V;
+    cx<T> *const acc_sm = acc_stage<T, THREADS, (FLAGS & K_ACC) != 0>();
+    if (FLAGS & K_ACC) {
+#pragma unroll
+        for (int k = 0; k < 12; ++k) cp_async_cx(acc_sm + k * THREADS + threadIdx.x, acc + k * V + s);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
 
     // accumulators start from the site-local terms (no loads are left for the epilogue)
     cx<T> hop[12];
@@ -204,7 +223,8 @@ __device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restri
             acc[k * V + s] = a;
         }
         if (FLAGS & K_ACC) {
-            cx<T> a = acc[k * V + s];
+            if (k == 0) cp_async_wait_all();
+            cx<T> a = acc_sm[k * THREADS + threadIdx.x];
             a.x = fma(sp.a_acc, w.x, a.x);
             a.y = fma(sp.a_acc, w.y, a.y);
             acc[k * V + s] = a;
