@@ -30,35 +30,41 @@ if ROOT not in sys.path:
 
 from paper_1510_06897_b200 import inputs, replicas  # noqa: E402
 
-WORKLOADS = {
-    # name: dims, link eps, stout steps, mu, degree, nev, eps of the polynomial (lower spectral edge / lambda_max)
-    "cfg3": dict(dims=(20, 20, 20, 64), link_eps=0.25, stout=3, mu=0.01, degree=400, nev=50, poly_eps=0.95 * 0.5 / 6.5,
-                 desc="BASELINE config 3: 20^3x64, U=exp(0.25iH)+3 stout rho=0.1, mu=0.01, degree 400, 50 deflation vectors"),
-    "cfg1": dict(dims=(8, 8, 8, 32), link_eps=0.3, stout=3, mu=0.01, degree=200, nev=20, poly_eps=0.95 * 0.505 / 6.5,
-                 desc="BASELINE config 1: 8^3x32, U=exp(0.3iH)+3 stout rho=0.1, mu=0.01, degree 200, 20 deflation vectors"),
-    "tiny": dict(dims=(4, 4, 4, 8), link_eps=0.3, stout=1, mu=0.01, degree=40, nev=4, poly_eps=0.09,
-                 desc="4^3x8 smoke-sized workload (not a benchmark)"),
-}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full` capture
-# (profiles/r1c_full.md: 682.1 MB with the psi term, 596.3 MB without, 198 : 199 launches per apply) -- bench.py cannot
-# run ncu itself; the value is reported only for the exact configuration that capture was taken on.
-NCU_TRAFFIC = {("cfg3", "f64", 18, "clenshaw"): {"bytes_per_launch": (198 * 682.1e6 + 199 * 596.3e6) / 397,
-                                                 "source": "profiles/r1c_full.md"}}
+WORKLOADS = inputs.WORKLOADS
+
+
+def csrc_hash():
+    """sha256 over the kernel sources and the boundary header: the key an ncu capture under profiles/ is valid for."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1510_06897_b200", "csrc")
+    for f in sorted(os.listdir(d)) + [os.path.join(ROOT, "include", "ovl.h")]:
+        with open(os.path.join(d, f) if not os.path.isabs(f) else f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full`
+    capture (profiles/traffic.json, written next to the capture it summarises).  bench.py cannot run ncu itself: the value
+    is reported only for the exact configuration AND kernel sources (csrc_hash) the capture was taken on, else null."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    except Exception:
+        return None, None
+    e = t.get(key)
+    if not e or e.get("csrc_hash") != csrc_hash():
+        return None, (f"stale: {e.get('source')} was captured on csrc {e.get('csrc_hash')}" if e else None)
+    return e["bytes_per_launch"], e["source"]
+
+
 METRIC = "overlap D[mu]psi applies/s"
 UNIT = "applies/s"
 
 
 def make_inputs(w, seed_off=0, need_phi=True):
     """Seeded synthetic stand-ins for the paper's ensembles (DESIGN.md input recipe)."""
-    dims = w["dims"]
-    k = {"cfg3": 3, "cfg1": 1, "tiny": 9}.get(w.get("name", ""), 7)
-    U = inputs.config_links(dims, w["link_eps"], inputs.SEED_BASE + k, stout_steps=w["stout"])
-    psi = inputs.gaussian_spinor(dims, inputs.SEED_BASE + 100 + k + 1000 * seed_off)
-    alpha = inputs.chebyshev_sign_coeffs(w["degree"], w["poly_eps"])
-    nev = w["nev"]
-    phi = inputs.phase_vectors(dims, nev, inputs.SEED_BASE + 200 + k) if (nev and need_phi) else None
-    lam = 0.5 * np.where(np.arange(nev) % 2 == 0, 1.0, -1.0) * (1.0 + 0.002 * np.arange(nev))
-    return U, psi, alpha, phi, lam
+    return inputs.workload_inputs(w, seed_off, need_phi)
 
 
 def poly_bytes(alpha, V, prec_bytes, recon, recurrence="clenshaw"):
@@ -173,47 +179,49 @@ def measured_peaks():
 
 # ------------------------------------------------------------------------------------------ reference arm (oracle)
 
-def oracle_overlap_rate(w, U, psi, alpha, phi, lam, sample_orders):
-    """Time the oracle (as it stands) on a bounded sample of the workload and extrapolate linearly in the number of
-    polynomial orders: T(full) = T(1 order + deflation) + [T(sample) - T(1 order)] * (orders - 1)/(sample - 1).
-    Returns (applies/s, threads, description, seconds spent)."""
+def oracle_full_apply(w, U, psi, alpha, phi, lam):
+    """One FULL oracle application y = D[mu] psi on the workload's inputs (every polynomial order, every deflation
+    vector), as the oracle stands.  Returns (y, seconds)."""
     from oracle import oracle as orc
-    dims = w["dims"]
-    last = max(m for m in range(1, len(alpha)) if alpha[m] != 0.0)
-    ns = min(sample_orders, last)
     t0 = time.perf_counter()
-    orc.overlap(dims, U, alpha[:2], w["mu"], psi, phi, lam)
-    t1 = time.perf_counter()
-    if ns > 1:
-        orc.overlap(dims, U, alpha[:ns + 1], w["mu"], psi, phi, lam)
-        t2 = time.perf_counter()
-        full = (t1 - t0) + ((t2 - t1) - (t1 - t0)) * (last - 1) / (ns - 1)
-    else:
-        t2 = t1
-        full = t1 - t0
-    full = max(full, 1e-9)
-    desc = (f"oracle overlap apply on the same inputs with the first {ns} of {last} polynomial orders plus the full "
-            f"{w['nev']}-vector deflation, extrapolated linearly in orders")
-    return 1.0 / full, orc.num_threads(), desc, t2 - t0
+    y = orc.overlap(w["dims"], U, alpha, w["mu"], psi, phi, lam)
+    return y, time.perf_counter() - t0
+
+
+def oracle_warm(w, U, psi, alpha, phi, lam, orders=8):
+    """Untimed warm-up of the oracle arm: a truncated apply (first `orders` polynomial orders + the full deflation) --
+    it touches every array and spins up the OpenMP team; the timed steps are full applies."""
+    from oracle import oracle as orc
+    orc.overlap(w["dims"], U, alpha[:orders + 1], w["mu"], psi, phi, lam)
 
 
 def run_reference(args, w):
+    """--impl reference: the CPU oracle on this box's host cores, same config / metric / unit as the native arm.  Every
+    timed step is one full apply (measured, not extrapolated); warm-up steps are truncated applies.  If K full applies
+    do not fit in --ref-budget-s the run stops early and reports the steps it actually timed."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    from oracle import oracle as orc
     U, psi, alpha, phi, lam = make_inputs(w)
-    rates, spent = [], 0.0
-    for i in range(args.warmup + args.steps):
-        r, cores, desc, dt = oracle_overlap_rate(w, U, psi, alpha, phi, lam, args.ref_orders)
-        spent += dt
-        if i >= args.warmup:
-            rates.append(r)
-    val = float(len(rates) / sum(1.0 / r for r in rates))
+    for _ in range(args.warmup):
+        oracle_warm(w, U, psi, alpha, phi, lam)
+    times, t_start = [], time.perf_counter()
+    for i in range(args.steps):
+        if times and (time.perf_counter() - t_start) + max(times) > args.ref_budget_s:
+            break
+        times.append(oracle_full_apply(w, U, psi, alpha, phi, lam)[1])
+    steps = len(times)
+    val = steps / sum(times)
+    last = max(m for m in range(1, len(alpha)) if alpha[m] != 0.0)
+    desc = (f"{steps} full oracle applies (all {last} polynomial orders + {w['nev']}-vector deflation each), measured; "
+            f"{args.warmup} warm-up steps were truncated 8-order applies"
+            + ("" if steps == args.steps else f"; {args.steps} steps were requested, the time budget of {args.ref_budget_s:.0f} s allowed {steps}"))
     line = {
-        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": args.warmup, "ms_per_step": 1e3 / val, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic", "config": {"workload": w["desc"], "precision": "f64", "links": "18-real"},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": desc},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -276,7 +284,7 @@ def dslash_sweep(torch, api, hbm_peak, reps=100):
 
 
 def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with_e2e, host_inputs=None,
-                  recurrence="clenshaw"):
+                  recurrence="clenshaw", keep_output=False):
     """Resident + end-to-end timing of one workload in one precision. Returns a dict of measurements."""
     U, psi, alpha, phi, lam = host_inputs if host_inputs is not None else make_inputs(w, seed_off=rank)
     dims, mu = w["dims"], w["mu"]
@@ -297,29 +305,34 @@ def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with
         for _ in range(warmup):
             op.overlap_native(nin, nout, mu)
         torch.cuda.synchronize()
-        poly_ms, poly_launches = [], 0
 
         def step():
             op.overlap_native(nin, nout, mu)
 
-        # per-step polynomial-loop timing is read back after the region (events are recorded inside the library)
+        # the polynomial loop of EVERY timed step is bracketed by its own event pair inside the library (ring of 64)
         l0 = op.launch_count()
+        op.set_profiling(True)  # restart the ring
         sampler = ClockSampler(torch.cuda.current_device()).start()
         ms = time_region(torch, op.stream, step, steps, dist)
         clocks = sampler.stop()
         l1 = op.launch_count()
-        pm, poly_launches = op.last_poly_timing()  # last step's loop
-        poly_ms.append(pm)
+        pms = op.poly_timings(min(steps, 64))
+        _, poly_launches = op.last_poly_timing()
+        pm = float(np.mean(pms))
         res.update(ms_per_step=ms / steps, applies_per_s=steps / (ms * 1e-3), launches=l1 - l0, clocks=clocks,
-                   orders=orders, poly_ms=pm, poly_launches=poly_launches)
+                   orders=orders, poly_ms=pm, poly_ms_min=float(min(pms)), poly_ms_max=float(max(pms)),
+                   poly_steps_sampled=len(pms), poly_launches=poly_launches)
         bytes_poly, _ = poly_bytes(alpha, V, pb, recon, recurrence)
         res["poly_bytes"] = bytes_poly
         res["kernel_us"] = 1e3 * pm / poly_launches
+        res["kernel_us_min"] = 1e3 * min(pms) / poly_launches
+        res["kernel_us_max"] = 1e3 * max(pms) / poly_launches
         res["achieved_gbs"] = bytes_poly / (pm * 1e-3) / 1e9
         res["bytes_per_site_per_order"] = bytes_poly / V / poly_launches
-        # sanity property at any size: D^dag = gamma5 D gamma5 is not needed here; check output is finite
-        y = op.from_native(nout)
+        y = op.from_native(nout)  # the output of the last timed step: compared with the oracle by the caller
         res["finite"] = bool(torch.isfinite(torch.view_as_real(y)).all().item())
+        if keep_output:
+            res["y_host"] = y.cpu().numpy().astype(np.complex128)
         if with_e2e:
             ph = torch.from_numpy(psi).to(op.cdtype).pin_memory()
             oh = torch.empty_like(ph).pin_memory()
@@ -459,7 +472,10 @@ def run_native(args, w):
     hbm_peak, peak_src = measured_peaks()
     host_inputs = make_inputs(w, seed_off=replicas.rhs_seed_offset(rank))
     main = bench_overlap(torch, api, B, w, args.prec, args.recon, args.steps, args.warmup, dist, rank, True, host_inputs,
-                         args.recurrence)
+                         args.recurrence, keep_output=True)
+    y_timed = main.pop("y_host")
+    tkey = f"{args.workload}/{args.prec}/{args.recon}/{args.recurrence}"
+    traffic, traffic_src = ncu_traffic(tkey)
     n = world
     value = n * main["applies_per_s"]
     line = {
@@ -478,10 +494,10 @@ def run_native(args, w):
         "roofline": {"bound": "hbm", "kernel": f"k_wilson_fused (one Chebyshev order per launch, {args.recurrence} recurrence)",
                      "achieved": main["achieved_gbs"], "peak": hbm_peak, "unit": "GB/s",
                      "frac": main["achieved_gbs"] / hbm_peak, "peak_source": peak_src,
-                     "traffic": (NCU_TRAFFIC.get((args.workload, args.prec, args.recon, args.recurrence)) or {}).get("bytes_per_launch"),
-                     "traffic_source": (NCU_TRAFFIC.get((args.workload, args.prec, args.recon, args.recurrence)) or {}).get("source"),
+                     "traffic": traffic, "traffic_source": traffic_src, "csrc_hash": csrc_hash(),
                      "algorithmic_bytes_per_launch": main["poly_bytes"] / main["poly_launches"],
-                     "kernel_us": main["kernel_us"], "launches_per_step": main["poly_launches"],
+                     "kernel_us": main["kernel_us"], "kernel_us_min": main["kernel_us_min"], "kernel_us_max": main["kernel_us_max"],
+                     "steps_sampled": main["poly_steps_sampled"], "launches_per_step": main["poly_launches"],
                      "algorithmic_bytes_per_site_per_launch": main["bytes_per_site_per_order"],
                      "frac_of_nominal_8TBs": main["achieved_gbs"] / 8000.0},
     }
@@ -519,9 +535,20 @@ def run_native(args, w):
                 "applies_per_s": ro["applies_per_s"], "achieved_gbs": ro["achieved_gbs"], "frac": ro["achieved_gbs"] / hbm_peak,
                 "kernel_us": ro["kernel_us"], "algorithmic_bytes_per_site_per_launch": ro["bytes_per_site_per_order"]}
         extras["dslash"] = dslash_sweep(torch, api, hbm_peak)
+        # the oracle, as it stands, on this box's host cores: ONE full apply on the timed inputs (measured, not extrapolated);
+        # its output is also the parity check of what the GPU arm just timed
+        from oracle import oracle as orc
         U, psi, alpha, phi, lam = host_inputs
-        r, cores, desc, _ = oracle_overlap_rate(w, U, psi, alpha, phi, lam, args.ref_orders)
-        line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        oracle_warm(w, U, psi, alpha, phi, lam)
+        y_ref, secs = oracle_full_apply(w, U, psi, alpha, phi, lam)
+        line["cpu_baseline"] = {"value": 1.0 / secs, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                                "sample": f"one full oracle apply on the timed inputs (all {main['orders']} orders + "
+                                          f"{w['nev']}-vector deflation), {secs:.1f} s measured"}
+        err = float(np.linalg.norm((y_timed - y_ref).ravel()) / np.linalg.norm(y_ref.ravel()))
+        tol = 1e-10 if args.prec == "f64" else 1e-5
+        extras["parity_vs_oracle_of_timed_output"] = {"rel_l2": err, "tol": tol, "ok": bool(err < tol)}
+        if not err < tol:
+            raise SystemExit(f"bench.py: the timed output disagrees with the oracle: rel L2 {err:.3e} >= {tol:g}")
     line["extras"] = extras
     if rank == 0:
         print(json.dumps(line))
@@ -540,7 +567,8 @@ def main():
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--recurrence", default="clenshaw", choices=["clenshaw", "forward"],
                     help="evaluation order of the polynomial sum of eq. 2.3 (ovl_set_recurrence)")
-    ap.add_argument("--ref-orders", type=int, default=12, help="polynomial orders in the oracle's bounded sample")
+    ap.add_argument("--ref-budget-s", type=float, default=330.0,
+                    help="--impl reference: stop timing full oracle applies once the next one would pass this many seconds")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--cfg3-eigensolver", action="store_true",
                     help="extras: also compute the 50 deflation pairs of config 3 on the GPU (ovl_lowest_eigenpairs, ~40 s)")
@@ -552,6 +580,16 @@ def main():
     if args.fast_inputs:
         w["stout"] = 0
         w["desc"] += " [--fast-inputs: links NOT smeared; profiling run]"
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # not under torchrun: launch the N ranks ourselves (one process per GPU, NCCL over 127.0.0.1)
+        import socket
+        import subprocess
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args, w)
     else:

@@ -184,6 +184,10 @@ int ovl_overlap_multi_native(ovl_ctx *ctx, int nrhs, double mu, int dagger, cons
  * those events and returns the loop's device time in ms and the number of fused-kernel launches in it. */
 int ovl_set_profiling(ovl_ctx *ctx, int on);
 int ovl_last_poly_timing(ovl_ctx *ctx, float *ms_out, int *launches_out);
+/* Loop times of the last min(max_n, 64, loops profiled since ovl_set_profiling) profiled polynomial loops, oldest first
+ * (one event pair per loop, kept in a ring of 64): ms_out[0..*n_out).  Synchronises those events.  OVL_ESTATE if no loop
+ * has been profiled yet. */
+int ovl_poly_timings(ovl_ctx *ctx, int max_n, float *ms_out, int *n_out);
 /* Total kernels this context has launched since creation (bench.py's gpu_launches). */
 long long ovl_launch_count(const ovl_ctx *ctx);
 

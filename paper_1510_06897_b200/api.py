@@ -155,5 +155,8 @@ class Overlap:
     def last_poly_timing(self):
         return B.ovl_last_poly_timing(self.ctx)
 
+    def poly_timings(self, max_n=64):
+        return B.ovl_poly_timings(self.ctx, max_n)
+
     def launch_count(self):
         return B.ovl_launch_count(self.ctx)

@@ -52,6 +52,7 @@ SIGNATURES = {
     "ovl_overlap_multi_native": (_I, [_P, _I, _D, _I, _P, _P]),
     "ovl_set_profiling": (_I, [_P, _I]),
     "ovl_last_poly_timing": (_I, [_P, C.POINTER(C.c_float), C.POINTER(_I)]),
+    "ovl_poly_timings": (_I, [_P, _I, C.POINTER(C.c_float), C.POINTER(_I)]),
     "ovl_launch_count": (C.c_longlong, [_P]),
 }
 
@@ -250,6 +251,13 @@ def ovl_last_poly_timing(ctx):
     ms, n = C.c_float(0.0), _I(0)
     _check(ctx, load_library().ovl_last_poly_timing(ctx, C.byref(ms), C.byref(n)))
     return float(ms.value), int(n.value)
+
+
+def ovl_poly_timings(ctx, max_n=64):
+    """Loop times (ms) of the last up-to-max_n profiled polynomial loops, oldest first."""
+    buf, n = (C.c_float * int(max_n))(), _I(0)
+    _check(ctx, load_library().ovl_poly_timings(ctx, int(max_n), buf, C.byref(n)))
+    return [float(buf[i]) for i in range(n.value)]
 
 
 def ovl_launch_count(ctx) -> int:

@@ -117,8 +117,10 @@ int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int pre
         OVL_CUDA(c, cudaMemsetAsync(c->sc_dev, 0, sizeof(double) * SC_N * OVL_MAX_RHS, c->st));
         OVL_CUDA(c, cudaMallocHost((void **)&c->sc_host, sizeof(double) * SC_N * OVL_MAX_RHS));
         OVL_CUDA(c, cudaMalloc((void **)&c->w_dev, sizeof(double2)));
-        OVL_CUDA(c, cudaEventCreate(&c->ev0));
-        OVL_CUDA(c, cudaEventCreate(&c->ev1));
+        for (int i = 0; i < ovl_ctx::NPROF; ++i) {
+            OVL_CUDA(c, cudaEventCreate(&c->pev0[i]));
+            OVL_CUDA(c, cudaEventCreate(&c->pev1[i]));
+        }
         // links: host pointers go through a temporary device copy of the canonical array
         const size_t cb = (size_t)c->g.V * 36 * sizeof(double2);
         const double2 *src = (const double2 *)links_c128;
@@ -153,8 +155,10 @@ int ovl_destroy(ovl_ctx *c) {
     for (auto &e : c->graphs)
         if (e.exec) cudaGraphExecDestroy(e.exec);
     if (c->sc_host) cudaFreeHost(c->sc_host);
-    if (c->ev0) cudaEventDestroy(c->ev0);
-    if (c->ev1) cudaEventDestroy(c->ev1);
+    for (int i = 0; i < ovl_ctx::NPROF; ++i) {
+        if (c->pev0[i]) cudaEventDestroy(c->pev0[i]);
+        if (c->pev1[i]) cudaEventDestroy(c->pev1[i]);
+    }
     cudaGetLastError();
     delete c;
     return OVL_OK;
@@ -376,15 +380,27 @@ int ovl_overlap_multi(ovl_ctx *c, int nrhs, double mu, int dagger, const void *p
 int ovl_set_profiling(ovl_ctx *c, int on) {
     if (!c) return OVL_EINVAL;
     c->profiling = on != 0;
-    c->poly_timed = false;
+    c->prof_count = 0;
     return OVL_OK;
 }
 int ovl_last_poly_timing(ovl_ctx *c, float *ms, int *launches) {
     if (!c || !ms || !launches) return OVL_EINVAL;
-    if (!c->poly_timed) return fail(c, OVL_ESTATE, "no profiled polynomial loop yet");
-    OVL_CUDA(c, cudaEventSynchronize(c->ev1));
-    OVL_CUDA(c, cudaEventElapsedTime(ms, c->ev0, c->ev1));
+    int n = 0;
+    OVL_TRY(ovl_poly_timings(c, 1, ms, &n));
     *launches = c->last_poly_launches;
+    return OVL_OK;
+}
+int ovl_poly_timings(ovl_ctx *c, int max_n, float *ms_out, int *n_out) {
+    if (!c || !ms_out || !n_out || max_n < 1) return OVL_EINVAL;
+    if (c->prof_count == 0) return fail(c, OVL_ESTATE, "no profiled polynomial loop yet");
+    long long n = c->prof_count < ovl_ctx::NPROF ? c->prof_count : ovl_ctx::NPROF;
+    if (n > max_n) n = max_n;
+    for (long long i = 0; i < n; ++i) {  // oldest of the last n first
+        const int slot = (int)((c->prof_count - n + i) % ovl_ctx::NPROF);
+        OVL_CUDA(c, cudaEventSynchronize(c->pev1[slot]));
+        OVL_CUDA(c, cudaEventElapsedTime(&ms_out[i], c->pev0[slot], c->pev1[slot]));
+    }
+    *n_out = (int)n;
     return OVL_OK;
 }
 long long ovl_launch_count(const ovl_ctx *c) { return c ? c->launches : 0; }

@@ -243,8 +243,9 @@ k_cg_scalars(int nblk, const double *__restrict__ partial, double *sc, int what,
     r = block_sum(r, sm);
     if (threadIdx.x == 0) {
         const bool frozen = sc[SC_FROZEN] != 0.0;
-        if (what == 0) { sc[SC_BB] = r; sc[SC_RR] = r; sc[SC_FROZEN] = 0.0; sc[SC_ALPHA] = 0.0; sc[SC_BETA] = 0.0; }
-        else if (what == 1) { sc[SC_PAP] = r; sc[SC_ALPHA] = frozen ? 0.0 : sc[SC_RR] / r; }
+        // a zero right-hand side is frozen from the start (x = 0 is its solution; 0/0 must not reach the vectors)
+        if (what == 0) { sc[SC_BB] = r; sc[SC_RR] = r; sc[SC_FROZEN] = r == 0.0 ? 1.0 : 0.0; sc[SC_ALPHA] = 0.0; sc[SC_BETA] = 0.0; }
+        else if (what == 1) { sc[SC_PAP] = r; sc[SC_ALPHA] = (frozen || r == 0.0) ? 0.0 : sc[SC_RR] / r; }
         else if (what == 2) {
             if (frozen) sc[SC_BETA] = 0.0;
             else {

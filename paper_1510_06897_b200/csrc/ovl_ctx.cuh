@@ -54,9 +54,10 @@ struct ovl_ctx {
 
     // measurement
     bool profiling = false;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    static constexpr int NPROF = 64;  // ring of event pairs: one per profiled polynomial loop
+    cudaEvent_t pev0[NPROF] = {}, pev1[NPROF] = {};
+    long long prof_count = 0;         // profiled loops since ovl_set_profiling(on)
     int last_poly_launches = 0;
-    bool poly_timed = false;
     long long launches = 0;
 
     char err[256] = {0};

@@ -266,6 +266,7 @@ inline int eig_lowest(ovl_ctx *c, int nev, double tol, int max_cycles, int degre
         }
         if (cycle >= max_cycles) break;
         ++cycle;
+        have_result = false;  // the next cycle overwrites w.Z (the Ritz vectors of a missed end game) with K^ W
         // filter: damp [a, 1] of K^2, a = top of the block
         const double a = std::min(sigma[m - 1], 0.95);
         const double cc = 0.5 * (1.0 + a), ee = 0.5 * (1.0 - a);

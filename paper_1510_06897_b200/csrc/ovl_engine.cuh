@@ -117,6 +117,9 @@ template <typename T> int cheb_clenshaw(ovl_ctx *c, const void *src, int nrhs) {
 }
 
 template <typename T> int cheb_launches(ovl_ctx *c, const void *src, int nrhs) {
+    // a table with alpha_m = 0 for all m >= 1 (reading R8: alpha_0 is honoured) has no K^ term to scale the Clenshaw
+    // launch by; the forward launch evaluates acc = alpha_0 src + 0 * K^ src without dividing by the hop coefficient
+    if (c->norders == 1 && c->alpha[1] == 0.0) return cheb_forward<T>(c, src, nrhs);
     return c->recurrence == OVL_REC_FORWARD ? cheb_forward<T>(c, src, nrhs) : cheb_clenshaw<T>(c, src, nrhs);
 }
 
@@ -165,14 +168,15 @@ template <typename T> int cheb_graph(ovl_ctx *c, const void *src, int nrhs, bool
 
 // acc = sum_{m=0}^{norders} alpha_m T_m(K^) src    (first sum of eq. 2.3; src is not modified)
 template <typename T> int cheb_native(ovl_ctx *c, const void *src, int nrhs) {
-    if (c->profiling) OVL_CUDA(c, cudaEventRecord(c->ev0, c->st));
+    const int pslot = (int)(c->prof_count % ovl_ctx::NPROF);
+    if (c->profiling) OVL_CUDA(c, cudaEventRecord(c->pev0[pslot], c->st));
     bool done = false;
     OVL_TRY(cheb_graph<T>(c, src, nrhs, &done));
     if (!done) OVL_TRY(cheb_launches<T>(c, src, nrhs));
     if (c->profiling) {
-        OVL_CUDA(c, cudaEventRecord(c->ev1, c->st));
+        OVL_CUDA(c, cudaEventRecord(c->pev1[pslot], c->st));
         c->last_poly_launches = c->norders;
-        c->poly_timed = true;
+        ++c->prof_count;
     }
     return OVL_OK;
 }

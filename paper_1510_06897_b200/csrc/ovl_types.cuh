@@ -47,7 +47,8 @@ struct Geom {
     int sxy, sxyz; // Lx*Ly, Lx*Ly*Lz
 };
 
-// read-only (non-coherent) loads: fields are never written by the kernel that stencil-reads them
+// read-only (non-coherent) loads, for the fields a kernel never writes (links, the stencil operand, psi, eigenvectors);
+// `prev` of the fused kernel may alias its output and is NOT read through this path
 __device__ __forceinline__ double2 ldg(const double2 *p) { return __ldg(p); }
 __device__ __forceinline__ float2 ldg(const float2 *p) { return __ldg(p); }
 

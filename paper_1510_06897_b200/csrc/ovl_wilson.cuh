@@ -9,7 +9,8 @@
 //                                                         or Clenshaw b_k = alpha_k psi + 2 K^ b_{k+1} - b_{k+2}
 //     w     += a_psi psi(x)                 [K_PSI]       the alpha_k psi term of the Clenshaw form
 //     out(x) = w                            [unless K_NOWRITE]  (may alias prev: prev[k,x] / out[k,x] are read then written by
-//                                                         the same thread with a true data dependency, so __restrict__ is safe)
+//                                                         the same thread with a true data dependency; prev is therefore read
+//                                                         with plain coherent loads and neither pointer is __restrict__)
 //     acc(x)+= a_acc w                      [K_ACC]       forward form: + alpha_{m+1} t_{m+1}
 //     acc(x) = a_init in(x) + a_acc w       [K_ACCI]      forward form, first order: alpha_0 t_0 + alpha_1 t_1
 // This is the paper's "merging together the Wilson matrix and polynomial algebra ... into a single GPU kernel"
@@ -160,7 +161,7 @@ template <typename T, int THREADS, bool ENABLE> __device__ __forceinline__ cx<T>
 // The kernel body for one tile of THREADS consecutive sites of one right-hand side.
 template <typename T, int RECON, int FLAGS, int THREADS>
 __device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in,
-                                            const cx<T> *__restrict__ prev, const cx<T> *__restrict__ psi, cx<T> *__restrict__ out,
+                                            const cx<T> *prev, const cx<T> *__restrict__ psi, cx<T> *out,
                                             cx<T> *__restrict__ acc, const StepParams<T> &sp, int tile) {
     const int s = tile * THREADS + threadIdx.x;
     if (s >= g.V) return;
@@ -187,7 +188,7 @@ __device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restri
     if (FLAGS & K_PREV) {
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const cx<T> pv = ldg(prev + k * V + s);
+            const cx<T> pv = prev[k * V + s];  // ld.global (not .nc): out may alias prev
             const T r = ((FLAGS & K_G5) && k >= 6) ? sp.r_p : -sp.r_p;
             hop[k].x = fma(r, pv.x, hop[k].x);
             hop[k].y = fma(r, pv.y, hop[k].y);
@@ -235,8 +236,8 @@ __device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restri
 // Single right-hand side: the field pointers stay kernel parameters (constant bank).
 template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *__restrict__ prev,
-               const cx<T> *__restrict__ psi, cx<T> *__restrict__ out, cx<T> *__restrict__ acc, const StepParams<T> sp) {
+k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *prev,
+               const cx<T> *__restrict__ psi, cx<T> *out, cx<T> *__restrict__ acc, const StepParams<T> sp) {
     const int tile = sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
     wilson_tile<T, RECON, FLAGS, THREADS>(g, U, in, prev, psi, out, acc, sp, tile);
 }

@@ -239,3 +239,39 @@ def phase_vectors(dims, nvec: int, seed: int) -> np.ndarray:
         ang = theta + (2.0 * np.pi * i / n) * e
         out[i] = (np.cos(ang) + 1j * np.sin(ang)) / np.sqrt(n)
     return out.reshape(nvec, volume(dims), 4, 3)
+
+
+# --------------------------------------------------------------------------------------
+# The BASELINE.json configurations as concrete seeded inputs; bench.py times exactly these
+# arrays and tests/test_gpu_configs.py holds the CUDA path against the oracle on them.
+# --------------------------------------------------------------------------------------
+
+WORKLOADS = {
+    # name: dims, link eps, stout steps, mu, degree, nev, eps of the polynomial (lower spectral edge / lambda_max)
+    "cfg3": dict(dims=(20, 20, 20, 64), link_eps=0.25, stout=3, mu=0.01, degree=400, nev=50, poly_eps=0.95 * 0.5 / 6.5, k=3,
+                 desc="BASELINE config 3: 20^3x64, U=exp(0.25iH)+3 stout rho=0.1, mu=0.01, degree 400, 50 deflation vectors"),
+    "cfg1": dict(dims=(8, 8, 8, 32), link_eps=0.3, stout=3, mu=0.01, degree=200, nev=20, poly_eps=0.95 * 0.505 / 6.5, k=1,
+                 desc="BASELINE config 1: 8^3x32, U=exp(0.3iH)+3 stout rho=0.1, mu=0.01, degree 200, 20 deflation vectors"),
+    "tiny": dict(dims=(4, 4, 4, 8), link_eps=0.3, stout=1, mu=0.01, degree=40, nev=4, poly_eps=0.09, k=9,
+                 desc="4^3x8 smoke-sized workload (not a benchmark)"),
+}
+CFG2_MU, CFG2_TOL, CFG2_SEED_OFF = 0.05, 1e-8, 7  # BASELINE config 2 = the cfg1 lattice, CG on D^dag D x = b
+
+
+def workload(name: str) -> dict:
+    return dict(WORKLOADS[name], name=name)
+
+
+def workload_inputs(w: dict, seed_off: int = 0, need_phi: bool = True):
+    """(U, psi, alpha, phi, lambda) of a workload: smeared seeded links, Gaussian right-hand side (seed_off selects
+    another one on the same links), the Chebyshev table, and nev exactly orthonormal deflation-shaped vectors with
+    prescribed eigenvalues of both signs near the lower spectral edge (reading R10: eq. 2.3 is a linear map for any
+    (phi_i, lambda_i); true eigenpairs at these volumes exist in closed form on pure-gauge links only, tests/closed_forms.py)."""
+    dims, k = w["dims"], w.get("k", 7)
+    U = config_links(dims, w["link_eps"], SEED_BASE + k, stout_steps=w["stout"])
+    psi = gaussian_spinor(dims, SEED_BASE + 100 + k + 1000 * seed_off)
+    alpha = chebyshev_sign_coeffs(w["degree"], w["poly_eps"])
+    nev = w["nev"]
+    phi = phase_vectors(dims, nev, SEED_BASE + 200 + k) if (nev and need_phi) else None
+    lam = 0.5 * np.where(np.arange(nev) % 2 == 0, 1.0, -1.0) * (1.0 + 0.002 * np.arange(nev))
+    return U, psi, alpha, phi, lam

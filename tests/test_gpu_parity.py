@@ -206,15 +206,15 @@ def test_config1_shape_8x8x8x32_degree200_nev20(torch, api, orc, rec):
     with api.Overlap(dims, dev(torch, U)) as op:
         op.set_recurrence(rec)
         assert op.set_chebyshev(alpha) == 199  # degree 200 table, alpha_200 = 0 (reading R7)
-        op.set_deflation(dev(torch, phi), lam)
         p = dev(torch, psi)
+        s2 = host(op.sign(op.sign(p)))  # before the stand-in vectors are set: the polynomial alone
+        op.set_deflation(dev(torch, phi), lam)
         got = host(op.overlap(p, 0.01))
-        s = op.sign(p)
-        s2 = host(op.sign(s))
     assert rel_err(got, want) < TOL_OVL
-    # sign^2 = 1 up to the polynomial error (the vectors are not eigenvectors, so only the undeflated bound applies
-    # on the complement; keep it loose)
-    assert np.isfinite(s2).all()
+    # sign^2 = 1 up to the polynomial error: ||s^2 psi - psi|| <= (2 delta + delta^2) ||psi|| (SURVEY §8(c) pins), delta =
+    # max |p - 1| on [eps, 1]; the stand-in vectors are not eigenvectors, so the bound is checked without them
+    delta = np.abs(inputs.chebyshev_eval(alpha, np.linspace(0.95 * 0.505 / 6.5, 1.0, 20001)) - 1.0).max()
+    assert rel_err(s2, psi) <= 2 * delta + delta * delta + 1e-12
 
 
 def test_cg_fixed_iterations_and_to_tolerance(torch, api, orc, dense44):
@@ -615,3 +615,53 @@ def test_deflation_exact_eigenpairs_4x4(torch, api, orc, dense44):
     assert rel_err(got, orc.sign(d["dims"], d["U"], alpha, psi, phi, lam_d).ravel()) < TOL_OVL
     exact = d["S"] @ psi.ravel()
     assert np.linalg.norm(got - exact) < np.linalg.norm(plain - exact)
+
+
+@pytest.mark.parametrize("rec", RECS)
+def test_table_with_only_alpha0(torch, api, orc, rec):
+    """alpha = [c0, 0]: no K^ term at all (reading R8: alpha_0 is honoured) -- sign() must return c0 psi, not NaN."""
+    dims = (4, 4, 4, 4)
+    U = inputs.random_links(dims, 0.5, 9)
+    psi = inputs.gaussian_spinor(dims, 10)
+    alpha = np.array([0.75, 0.0])
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_recurrence(rec)
+        assert op.set_chebyshev(alpha) == 1
+        got = host(op.sign(dev(torch, psi)))
+    assert rel_err(got, orc.sign(dims, U, alpha, psi)) < TOL_OVL
+    assert rel_err(got, 0.75 * psi) < 1e-14
+
+
+def test_cg_multi_with_a_zero_right_hand_side(torch, api, orc):
+    """One zero source among several: its solution is exactly 0 (no NaN from 0/0) and the others are untouched."""
+    dims = (4, 4, 4, 8)
+    U = inputs.config_links(dims, 0.3, 77, stout_steps=1)
+    alpha = inputs.chebyshev_sign_coeffs(41, 0.09)
+    b = np.stack([inputs.gaussian_spinor(dims, 79), np.zeros((int(np.prod(dims)), 4, 3), complex), inputs.gaussian_spinor(dims, 81)])
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        bd = dev(torch, b)
+        x, its, rels, ok = op.cg_multi(bd, 0.2, tol=1e-9, maxiter=500)
+        assert ok and its[1] == 0 and rels[1] == 0.0
+        assert torch.count_nonzero(x[1]).item() == 0
+        for r in (0, 2):
+            xs, it1, _, ok1 = op.cg(bd[r].contiguous(), 0.2, tol=1e-9, maxiter=500)
+            assert ok1 and it1 == its[r] and torch.equal(xs, x[r])
+        x0, it0, rel0, ok0 = op.cg(bd[1].contiguous(), 0.2, tol=1e-9, maxiter=50)
+        assert ok0 and it0 == 0 and torch.count_nonzero(x0).item() == 0
+
+
+def test_eigensolver_not_converged_returns_consistent_ritz_pairs(torch, api, orc):
+    """OVL_ENOTCONV path: with too few cycles the returned (phi_i, lambda_i, resid_i) must still belong together --
+    ||K phi_i - lambda_i phi_i|| recomputed with the oracle's K equals the reported residual."""
+    dims = (4, 4, 4, 8)
+    U = inputs.config_links(dims, 0.3, 61, stout_steps=1)
+    with api.Overlap(dims, dev(torch, U)) as op:
+        for cycles, tol in [(1, 1e-13), (2, 1e-9), (3, 1e-11)]:
+            phi, lam, res, cyc, ok = op.lowest_eigenpairs(4, tol=tol, max_cycles=cycles, filter_degree=6, block=6)
+            ph = host(phi)
+            for i in range(4):
+                kp = 6.5 * orc.khat(dims, U, ph[i])
+                r = np.linalg.norm((kp - lam[i] * ph[i]).ravel())
+                assert abs(r - res[i]) <= 1e-9 + 1e-6 * res[i], (cycles, i, r, res[i], ok)
+                assert abs(np.linalg.norm(ph[i].ravel()) - 1.0) < 1e-10
