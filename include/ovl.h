@@ -30,8 +30,9 @@
  *   cudaPointerGetAttributes.  `alpha`, `lambda`, `dims` and the scalar out-parameters are host memory.
  *
  * Ownership.  The caller owns everything it passes in; the library never frees or keeps caller pointers.  Links and
- *   eigenvectors are re-laid-out into context-owned device memory (cudaMalloc) at create / set time, so the
- *   caller may release them afterwards.  `out` must not alias `psi`.
+ *   eigenvectors are re-laid-out into the context's device memory -- the caller's workspace (ovl_create_ws) or
+ *   library allocations (ovl_create) -- at create / set time, so the caller may release them afterwards.  `out` must
+ *   not alias `psi`.
  *
  * Execution.  All work is enqueued on the stream given to ovl_create.  Calls with device outputs return without
  *   synchronising; ovl_cg, ovl_destroy and any call with a host output synchronise the stream.  A context is
@@ -60,21 +61,39 @@ enum { OVL_REC_CLENSHAW = 0, OVL_REC_FORWARD = 1 }; /* how sum_m alpha_m T_m(K^)
 /* Library version string, e.g. "ovl-b200 0.1 (sm_100a)". */
 const char *ovl_version(void);
 
-/* Device bytes a context for this configuration allocates (links + work vectors + max_nev eigenvectors) when it is used
- * with one right-hand side at a time.  On top of that: ovl_overlap_multi / ovl_cg_multi grow the recurrence and CG
- * workspaces to nrhs fields each (8 * (nrhs - 1) more fields, kept until ovl_destroy), ovl_cg allocates its 4 vectors on
- * first use, and ovl_lowest_eigenpairs needs 4 * max(block, 2 nev) + 2 nev fields while it runs. */
+/* Device bytes of the workspace a context needs for: this lattice / precision / link storage, up to max_nev deflation
+ * vectors, up to max_rhs right-hand sides per ovl_overlap_multi / ovl_cg_multi call (1..OVL_MAX_RHS) and an
+ * ovl_lowest_eigenpairs work block of eig_block = max(block, 2 nev) vectors (0: the eigensolver is not used; <= 128).
+ * It holds the re-laid-out links, the recurrence vectors (S4: "short three vector recurrence"), the CG vectors,
+ * the multi-right-hand-side staging, the eigenvector store (S5), the canonical staging for host pointers, the reduction
+ * scratch and the eigensolver block.  0 for invalid arguments. */
+size_t ovl_workspace_bytes(const int dims[4], int prec, int recon, int max_nev, int max_rhs, int eig_block);
+/* = ovl_workspace_bytes(dims, prec, recon, max_nev, 1, 0). */
 size_t ovl_device_bytes(const int dims[4], int prec, int recon, int max_nev);
 
-/* Create a context: re-lay-out the links (S2; SoA site-coalesced planes, optional 12-real compression) and
- * allocate the recurrence workspace (S4: "short three vector recurrence").
- *   links_c128 [H|D]  canonical links, V*4*9 complex128.
+/* Create a context inside a CALLER-OWNED workspace (PyTorch owns device memory): `workspace` is device
+ * memory of at least ovl_workspace_bytes(...) bytes for the same capacities, 256-byte aligned, and must stay valid until
+ * ovl_destroy, which does not free it.  Every device buffer of the context is carved from it here; NO later call
+ * allocates or frees device memory (calls that exceed a capacity -- nev > max_nev, nrhs > max_rhs, an eigensolver block
+ * above eig_block -- return OVL_EINVAL), so no call hides a device-wide synchronisation behind an allocation.
+ * Links are re-laid-out (S2; SoA site-coalesced planes, optional 12-real compression) before the call returns.
+ *   links_c128 [H|D]  canonical links, V*4*9 complex128 (a host array is staged through the workspace).
  *   cuda_stream       a cudaStream_t (0 = legacy default stream); all later work is enqueued there.
  * Defaults: m_w = 1.5, lambda_max = 8 - m_w = 6.5 (reading R5); no polynomial, no deflation.
+ * Errors: OVL_EINVAL (null / misaligned / non-device / too small workspace, extent < 2, unknown prec/recon, capacities
+ * out of range), OVL_ECUDA. */
+int ovl_create_ws(ovl_ctx **out, const int dims[4], const void *links_c128, int prec, int recon, int max_nev, int max_rhs,
+                  int eig_block, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Convenience: the same context with LIBRARY-owned memory.  One cudaMalloc here for the base set (links, recurrence
+ * vectors, reduction scratch = ovl_device_bytes(dims, prec, recon, 0) minus the optional parts); further allocations
+ * happen only when a capacity is first needed or grows: ovl_set_deflation (eigenvector store), the first ovl_cg*, the
+ * first multi-right-hand-side call with a larger nrhs, the first host-pointer call (staging), ovl_lowest_eigenpairs
+ * (work block, released on return).  Use ovl_create_ws when allocations inside calls are not acceptable.
  * Errors: OVL_EINVAL (null pointer, extent < 2, unknown prec/recon), OVL_ENOMEM, OVL_ECUDA. */
 int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int prec, int recon, void *cuda_stream);
 
-/* Synchronise the stream and free everything the context owns. */
+/* Synchronise the stream and free everything the library allocated (never the caller's workspace). */
 int ovl_destroy(ovl_ctx *ctx);
 
 /* K = gamma5 (D_W - m_w), K^ = K / lambda_max (R5).  lambda_max > 0. */

@@ -19,7 +19,11 @@ class Overlap:
     Spinors: (V,4,3) complex128 for prec='f64', complex64 for prec='f32'.
     """
 
-    def __init__(self, dims, links, prec="f64", recon=18, stream=None, m_w=1.5, lambda_max=6.5):
+    def __init__(self, dims, links, prec="f64", recon=18, stream=None, m_w=1.5, lambda_max=6.5, workspace=None):
+        """workspace: None -> the library allocates its own device memory (ovl_create); a dict(max_nev=, max_rhs=,
+        eig_block=) -> a torch-owned uint8 buffer of ovl_workspace_bytes is allocated here and the context lives in it
+        (ovl_create_ws: no cudaMalloc / cudaFree inside any later call); a CUDA uint8 tensor with the dict under
+        workspace["buffer"] is used as given."""
         torch = _torch()
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1510_06897_b200 needs a CUDA device (no CPU fallback)")
@@ -28,7 +32,18 @@ class Overlap:
         self.prec = B.OVL_F64 if prec in ("f64", B.OVL_F64) else B.OVL_F32
         self.recon = int(recon)
         self.stream = stream if stream is not None else torch.cuda.current_stream()
-        self.ctx = B.ovl_create(self.dims, links, self.prec, self.recon, self.stream.cuda_stream)
+        self.workspace = None
+        if workspace is None:
+            self.ctx = B.ovl_create(self.dims, links, self.prec, self.recon, self.stream.cuda_stream)
+        else:
+            caps = dict(max_nev=int(workspace.get("max_nev", 0)), max_rhs=int(workspace.get("max_rhs", 1)),
+                        eig_block=int(workspace.get("eig_block", 0)))
+            need = B.ovl_workspace_bytes(self.dims, self.prec, self.recon, **caps)
+            buf = workspace.get("buffer")
+            if buf is None:
+                buf = torch.empty(need, dtype=torch.uint8, device="cuda")
+            self.workspace, self.workspace_bytes = buf, need
+            self.ctx = B.ovl_create_ws(self.dims, links, buf, self.prec, self.recon, stream=self.stream.cuda_stream, **caps)
         B.ovl_set_kernel(self.ctx, m_w, lambda_max)
         self.cdtype = torch.complex128 if self.prec == B.OVL_F64 else torch.complex64
 

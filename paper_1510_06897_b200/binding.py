@@ -24,7 +24,9 @@ LIB_PATH = os.path.join(_HERE, "libovl.so")
 _P, _I, _D = C.c_void_p, C.c_int, C.c_double
 SIGNATURES = {
     "ovl_version": (C.c_char_p, []),
+    "ovl_workspace_bytes": (C.c_size_t, [C.POINTER(_I), _I, _I, _I, _I, _I]),
     "ovl_device_bytes": (C.c_size_t, [C.POINTER(_I), _I, _I, _I]),
+    "ovl_create_ws": (_I, [C.POINTER(_P), C.POINTER(_I), _P, _I, _I, _I, _I, _I, _P, C.c_size_t, _P]),
     "ovl_create": (_I, [C.POINTER(_P), C.POINTER(_I), _P, _I, _I, _P]),
     "ovl_destroy": (_I, [_P]),
     "ovl_set_kernel": (_I, [_P, _D, _D]),
@@ -116,6 +118,21 @@ def ovl_version() -> str:
 
 def ovl_device_bytes(dims, prec=OVL_F64, recon=OVL_RECON18, max_nev=0) -> int:
     return int(load_library().ovl_device_bytes((_I * 4)(*map(int, dims)), prec, recon, max_nev))
+
+
+def ovl_workspace_bytes(dims, prec=OVL_F64, recon=OVL_RECON18, max_nev=0, max_rhs=1, eig_block=0) -> int:
+    return int(load_library().ovl_workspace_bytes((_I * 4)(*map(int, dims)), prec, recon, max_nev, max_rhs, eig_block))
+
+
+def ovl_create_ws(dims, links, workspace, prec=OVL_F64, recon=OVL_RECON18, max_nev=0, max_rhs=1, eig_block=0, stream=0):
+    """Context inside a caller-owned device workspace (a torch uint8 CUDA tensor of >= ovl_workspace_bytes bytes)."""
+    ctx = _P()
+    nbytes = workspace.numel() * workspace.element_size()
+    rc = load_library().ovl_create_ws(C.byref(ctx), (_I * 4)(*map(int, dims)), _ptr(links), prec, recon, max_nev, max_rhs,
+                                      eig_block, _ptr(workspace), nbytes, _P(int(stream)))
+    if rc != OVL_OK:
+        raise OvlError(rc, "ovl_create_ws failed (bad workspace / arguments)")
+    return ctx
 
 
 def ovl_create(dims, links, prec=OVL_F64, recon=OVL_RECON18, stream=0):

@@ -69,6 +69,20 @@ template <typename T> int import_phi_t(ovl_ctx *c, const double2 *src_dev, int i
     return OVL_OK;
 }
 
+// native staging of the multi-right-hand-side calls with canonical arguments
+int ensure_multi_staging(ovl_ctx *c, int nrhs) {
+    if (nrhs <= c->multi_cap) return OVL_OK;
+    if (c->ws_mode) return fail(c, OVL_EINVAL, "%d right-hand sides exceed the workspace capacity max_rhs = %d", nrhs, c->max_rhs);
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    dev_release(c, &c->multi_in);
+    dev_release(c, &c->multi_out);
+    c->multi_cap = 0;
+    OVL_TRY(dev_alloc(c, &c->multi_in, c->field_bytes() * nrhs));
+    OVL_TRY(dev_alloc(c, &c->multi_out, c->field_bytes() * nrhs));
+    c->multi_cap = nrhs;
+    return OVL_OK;
+}
+
 // canonical in -> native psi_n, run `body(psi_n, out_n)`, native out_n -> canonical out
 template <typename F> int with_canonical(ovl_ctx *c, const void *psi, void *out, F body) {
     if (!c) return OVL_EINVAL;
@@ -78,25 +92,39 @@ template <typename F> int with_canonical(ovl_ctx *c, const void *psi, void *out,
     return export_any(c, c->out_n, out);
 }
 
-}  // namespace
 
-extern "C" {
-
-const char *ovl_version(void) { return "ovl-b200 0.2 (sm_100a)"; }
-
-size_t ovl_device_bytes(const int dims[4], int prec, int recon, int max_nev) {
-    if (check_cfg(dims, prec, recon) != OVL_OK || max_nev < 0) return 0;
-    const size_t V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
-    const size_t ts = prec == OVL_F64 ? 8 : 4;
-    const size_t field = V * 12 * 2 * ts;
-    const size_t links = V * 4 * (recon == OVL_RECON18 ? 9 : 6) * 2 * ts;
-    return links + field * (6 + 4 + (size_t)max_nev) + 2 * V * 12 * 16;
+// ---- the device-memory plan of a context (the caller owns the workspace).  One routine enumerates every
+// buffer in a fixed order; ovl_workspace_bytes sums it and create_impl carves it, so the two cannot disagree.
+struct WsGeom { size_t V; };
+WsGeom ws_geom(const int dims[4]) { return WsGeom{(size_t)dims[0] * dims[1] * dims[2] * dims[3]}; }
+enum WsId { WS_U, WS_PSI, WS_OUT, WS_TA, WS_TB, WS_ACC, WS_G5B, WS_RED, WS_SC, WS_W, WS_CG_R, WS_CG_P, WS_CG_Q, WS_CG_AP,
+            WS_MULTI_IN, WS_MULTI_OUT, WS_PHI, WS_PROJ, WS_COEF, WS_STAGE_IN, WS_STAGE_OUT, WS_EIG };
+size_t eig_ws_bytes(size_t V, int cap) { return eig_ws_total(V, cap); }  // ovl_eigsolve.cuh's work block for `cap` vectors
+template <typename F> void ws_visit(WsGeom g, int prec, int recon, int max_nev, int max_rhs, int eig_cap, F f) {
+    const size_t ts = prec == OVL_F64 ? 8 : 4, n = 12 * g.V, fb = n * 2 * ts;
+    const size_t red_nblk = grid_for(n, BLAS_THREADS * 4, 148 * 8), proj_nblk = (n + BLAS_THREADS * PROJ_EPT - 1) / (BLAS_THREADS * PROJ_EPT);
+    f(WS_U, g.V * 4 * (recon == OVL_RECON18 ? 9 : 6) * 2 * ts);
+    // psi_n .. g5b are contiguous and come first after the links: the canonical link array (36 V complex128) is staged there
+    // during ovl_create when the links are passed as a host pointer
+    f(WS_PSI, fb); f(WS_OUT, fb);
+    f(WS_TA, fb * max_rhs); f(WS_TB, fb * max_rhs); f(WS_ACC, fb * max_rhs); f(WS_G5B, fb * max_rhs);
+    f(WS_RED, sizeof(double) * red_nblk * OVL_MAX_RHS);
+    f(WS_SC, sizeof(double) * SC_N * OVL_MAX_RHS);
+    f(WS_W, sizeof(double2) * (max_nev > 0 ? max_nev : 1) * OVL_MAX_RHS);
+    // everything below is optional for a library-owned context (allocated on first use); a workspace holds all of it
+    f(WS_CG_R, fb * max_rhs); f(WS_CG_P, fb * max_rhs); f(WS_CG_Q, fb * max_rhs); f(WS_CG_AP, fb * max_rhs);
+    if (max_rhs > 1) { f(WS_MULTI_IN, fb * max_rhs); f(WS_MULTI_OUT, fb * max_rhs); }
+    if (max_nev > 0) {
+        f(WS_PHI, fb * max_nev);
+        f(WS_PROJ, sizeof(double2) * proj_nblk * max_nev * max_rhs);
+        f(WS_COEF, sizeof(double) * max_nev);
+    }
+    f(WS_STAGE_IN, n * sizeof(double2)); f(WS_STAGE_OUT, n * sizeof(double2));
+    if (eig_cap > 0) f(WS_EIG, eig_ws_bytes(g.V, eig_cap));
 }
 
-int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int prec, int recon, void *cuda_stream) {
-    if (!out) return OVL_EINVAL;
-    *out = nullptr;
-    if (!links_c128 || check_cfg(dims, prec, recon) != OVL_OK) return OVL_EINVAL;
+int create_impl(ovl_ctx **out, const int dims[4], const void *links_c128, int prec, int recon, void *cuda_stream, void *ws,
+                size_t ws_bytes, int max_nev, int max_rhs, int eig_cap) {
     ovl_ctx *c = new (std::nothrow) ovl_ctx();
     if (!c) return OVL_ENOMEM;
     for (int i = 0; i < 4; ++i) c->g.L[i] = dims[i];
@@ -106,34 +134,79 @@ int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int pre
     c->prec = prec;
     c->recon = recon;
     c->st = (cudaStream_t)cuda_stream;
+    c->red_nblk = grid_for(c->n(), BLAS_THREADS * 4, 148 * 8);
+    c->proj_nblk = (int)((c->n() + BLAS_THREADS * PROJ_EPT - 1) / (BLAS_THREADS * PROJ_EPT));
     auto body = [&]() -> int {
-        const size_t fb = c->field_bytes();
-        OVL_TRY(dev_alloc(c, &c->U, c->link_bytes()));
-        void **bufs[] = {&c->psi_n, &c->out_n, &c->tA, &c->tB, &c->acc, &c->g5b};
-        for (void **b : bufs) OVL_TRY(dev_alloc(c, b, fb));
-        c->red_nblk = grid_for(c->n(), BLAS_THREADS * 4, 148 * 8);
-        OVL_CUDA(c, cudaMalloc((void **)&c->red_partial, sizeof(double) * c->red_nblk * OVL_MAX_RHS));
-        OVL_CUDA(c, cudaMalloc((void **)&c->sc_dev, sizeof(double) * SC_N * OVL_MAX_RHS));
+        const WsGeom wg = ws_geom(dims);
+        if (ws) {  // caller-owned: carve everything now, never allocate again
+            c->ws_mode = true;
+            c->arena.base = (char *)ws; c->arena.size = ws_bytes;
+            c->max_nev = max_nev; c->max_rhs = max_rhs; c->eig_cap = eig_cap;
+        } else {   // library-owned: ONE cudaMalloc for the base set (links + recurrence vectors + reduction scratch)
+            size_t base = 0;
+            ws_visit(wg, prec, recon, 0, 1, 0, [&](int id, size_t b) { if (id <= WS_W) base += ws_round(b ? b : 16); });
+            void *p = nullptr;
+            OVL_CUDA(c, cudaMalloc(&p, base));
+            c->owned.push_back(p);
+            c->arena.base = (char *)p; c->arena.size = base;
+        }
+        int rc = OVL_OK;
+        ws_visit(wg, prec, recon, max_nev, max_rhs, eig_cap, [&](int id, size_t b) {
+            if (rc != OVL_OK || (!ws && id > WS_W)) return;
+            void **slot = nullptr;
+            switch (id) {
+                case WS_U: slot = &c->U; break;
+                case WS_PSI: slot = &c->psi_n; break;
+                case WS_OUT: slot = &c->out_n; break;
+                case WS_TA: slot = &c->tA; break;
+                case WS_TB: slot = &c->tB; break;
+                case WS_ACC: slot = &c->acc; break;
+                case WS_G5B: slot = &c->g5b; break;
+                case WS_RED: slot = (void **)&c->red_partial; break;
+                case WS_SC: slot = (void **)&c->sc_dev; break;
+                case WS_W: slot = (void **)&c->w_dev; break;
+                case WS_CG_R: slot = &c->cg_r; break;
+                case WS_CG_P: slot = &c->cg_p; break;
+                case WS_CG_Q: slot = &c->cg_q; break;
+                case WS_CG_AP: slot = &c->cg_Ap; break;
+                case WS_MULTI_IN: slot = &c->multi_in; break;
+                case WS_MULTI_OUT: slot = &c->multi_out; break;
+                case WS_PHI: slot = &c->phi; break;
+                case WS_PROJ: slot = (void **)&c->proj_partial; break;
+                case WS_COEF: slot = (void **)&c->coef_dev; break;
+                case WS_STAGE_IN: slot = &c->stage_in; break;
+                case WS_STAGE_OUT: slot = &c->stage_out; break;
+                case WS_EIG: slot = &c->eig_ws; c->eig_ws_bytes = b; break;
+            }
+            rc = dev_alloc(c, slot, b);
+        });
+        if (rc != OVL_OK) return rc;
+        c->work_nrhs = max_rhs;
+        if (ws) {
+            c->cg_nrhs = max_rhs;
+            c->multi_cap = max_rhs > 1 ? max_rhs : 0;
+            c->proj_cap = max_nev;
+            c->proj_rhs = max_rhs;
+        }
         OVL_CUDA(c, cudaMemsetAsync(c->sc_dev, 0, sizeof(double) * SC_N * OVL_MAX_RHS, c->st));
-        OVL_CUDA(c, cudaMallocHost((void **)&c->sc_host, sizeof(double) * SC_N * OVL_MAX_RHS));
-        OVL_CUDA(c, cudaMalloc((void **)&c->w_dev, sizeof(double2)));
+        OVL_CUDA(c, cudaMallocHost((void **)&c->sc_host, sizeof(double) * 2 * SC_N * OVL_MAX_RHS));
+        for (int i = 0; i < 2; ++i) OVL_CUDA(c, cudaEventCreateWithFlags(&c->cg_ev[i], cudaEventDisableTiming));
         for (int i = 0; i < ovl_ctx::NPROF; ++i) {
             OVL_CUDA(c, cudaEventCreate(&c->pev0[i]));
             OVL_CUDA(c, cudaEventCreate(&c->pev1[i]));
         }
-        // links: host pointers go through a temporary device copy of the canonical array
+        // links: a host array is staged through the (still unused) recurrence vectors, which start at psi_n and are
+        // contiguous: 6 fields >= 576 V bytes = the canonical link array in either precision
         const size_t cb = (size_t)c->g.V * 36 * sizeof(double2);
         const double2 *src = (const double2 *)links_c128;
-        void *tmp = nullptr;
         if (!is_device_ptr(links_c128)) {
-            OVL_CUDA(c, cudaMalloc(&tmp, cb));
-            cudaError_t e = cudaMemcpyAsync(tmp, links_c128, cb, cudaMemcpyHostToDevice, c->st);
-            if (e != cudaSuccess) { cudaFree(tmp); return fail(c, OVL_ECUDA, "link upload: %s", cudaGetErrorString(e)); }
-            src = (const double2 *)tmp;
+            if ((size_t)((char *)c->g5b + c->field_bytes() * max_rhs - (char *)c->psi_n) < cb)
+                return fail(c, OVL_ENOMEM, "internal: link staging area too small");
+            OVL_CUDA(c, cudaMemcpyAsync(c->psi_n, links_c128, cb, cudaMemcpyHostToDevice, c->st));
+            src = (const double2 *)c->psi_n;
         }
-        int rc = DISPATCH(c, import_links_t, c, src);
+        rc = DISPATCH(c, import_links_t, c, src);
         cudaError_t e = cudaStreamSynchronize(c->st);
-        if (tmp) cudaFree(tmp);
         if (rc != OVL_OK) return rc;
         if (e != cudaSuccess) return fail(c, OVL_ECUDA, "link import: %s", cudaGetErrorString(e));
         return OVL_OK;
@@ -144,17 +217,50 @@ int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int pre
     return OVL_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+const char *ovl_version(void) { return "ovl-b200 0.2 (sm_100a)"; }
+
+size_t ovl_workspace_bytes(const int dims[4], int prec, int recon, int max_nev, int max_rhs, int eig_block) {
+    if (check_cfg(dims, prec, recon) != OVL_OK || max_nev < 0 || max_rhs < 1 || max_rhs > OVL_MAX_RHS || eig_block < 0 || eig_block > 128) return 0;
+    size_t total = 0;
+    ws_visit(ws_geom(dims), prec, recon, max_nev, max_rhs, eig_block, [&](int, size_t b) { total += ws_round(b ? b : 16); });
+    return total;
+}
+
+size_t ovl_device_bytes(const int dims[4], int prec, int recon, int max_nev) {
+    return ovl_workspace_bytes(dims, prec, recon, max_nev, 1, 0);
+}
+
+int ovl_create_ws(ovl_ctx **out, const int dims[4], const void *links_c128, int prec, int recon, int max_nev, int max_rhs,
+                  int eig_block, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+    if (!out) return OVL_EINVAL;
+    *out = nullptr;
+    if (!links_c128 || !workspace || check_cfg(dims, prec, recon) != OVL_OK) return OVL_EINVAL;
+    const size_t need = ovl_workspace_bytes(dims, prec, recon, max_nev, max_rhs, eig_block);
+    if (need == 0 || workspace_bytes < need || ((uintptr_t)workspace % WS_ALIGN) != 0 || !is_device_ptr(workspace)) return OVL_EINVAL;
+    return create_impl(out, dims, links_c128, prec, recon, cuda_stream, workspace, workspace_bytes, max_nev, max_rhs, eig_block);
+}
+
+int ovl_create(ovl_ctx **out, const int dims[4], const void *links_c128, int prec, int recon, void *cuda_stream) {
+    if (!out) return OVL_EINVAL;
+    *out = nullptr;
+    if (!links_c128 || check_cfg(dims, prec, recon) != OVL_OK) return OVL_EINVAL;
+    return create_impl(out, dims, links_c128, prec, recon, cuda_stream, nullptr, 0, 0, 1, 0);
+}
+
 int ovl_destroy(ovl_ctx *c) {
     if (!c) return OVL_EINVAL;
     cudaStreamSynchronize(c->st);
-    void *bufs[] = {c->U, c->phi, c->psi_n, c->out_n, c->tA, c->tB, c->acc, c->g5b, c->cg_r, c->cg_p, c->cg_q, c->cg_Ap,
-                    c->stage_in, c->stage_out, c->proj_partial, c->w_dev, c->coef_dev, c->red_partial, c->sc_dev,
-                    c->multi_in, c->multi_out};
-    for (void *b : bufs)
+    for (void *b : c->owned)   // library-owned allocations only: a caller-owned workspace is never freed
         if (b) cudaFree(b);
     for (auto &e : c->graphs)
         if (e.exec) cudaGraphExecDestroy(e.exec);
     if (c->sc_host) cudaFreeHost(c->sc_host);
+    for (int i = 0; i < 2; ++i)
+        if (c->cg_ev[i]) cudaEventDestroy(c->cg_ev[i]);
     for (int i = 0; i < ovl_ctx::NPROF; ++i) {
         if (c->pev0[i]) cudaEventDestroy(c->pev0[i]);
         if (c->pev1[i]) cudaEventDestroy(c->pev1[i]);
@@ -216,17 +322,17 @@ int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda
     c->nev = 0;
     if (nev == 0) return OVL_OK;
     if (nev > c->proj_cap) {
-        if (c->phi) cudaFree(c->phi);
-        if (c->proj_partial) cudaFree(c->proj_partial);
-        if (c->w_dev) cudaFree(c->w_dev);
-        if (c->coef_dev) cudaFree(c->coef_dev);
-        c->phi = nullptr; c->proj_partial = nullptr; c->w_dev = nullptr; c->coef_dev = nullptr;
+        if (c->ws_mode) return fail(c, OVL_EINVAL, "%d eigenvectors exceed the workspace capacity max_nev = %d", nev, c->max_nev);
+        dev_release(c, &c->phi);
+        dev_release(c, (void **)&c->proj_partial);
+        dev_release(c, (void **)&c->w_dev);
+        dev_release(c, (void **)&c->coef_dev);
         c->proj_cap = 0;
-        c->proj_nblk = (int)((c->n() + BLAS_THREADS * PROJ_EPT - 1) / (BLAS_THREADS * PROJ_EPT));
-        OVL_CUDA(c, cudaMalloc(&c->phi, c->field_bytes() * nev));
-        OVL_CUDA(c, cudaMalloc((void **)&c->proj_partial, sizeof(double2) * (size_t)c->proj_nblk * nev));
-        OVL_CUDA(c, cudaMalloc((void **)&c->w_dev, sizeof(double2) * nev * OVL_MAX_RHS));
-        OVL_CUDA(c, cudaMalloc((void **)&c->coef_dev, sizeof(double) * nev));
+        OVL_TRY(dev_alloc(c, &c->phi, c->field_bytes() * nev));
+        c->proj_rhs = c->work_nrhs;
+        OVL_TRY(dev_alloc(c, (void **)&c->proj_partial, sizeof(double2) * (size_t)c->proj_nblk * nev * c->proj_rhs));
+        OVL_TRY(dev_alloc(c, (void **)&c->w_dev, sizeof(double2) * nev * OVL_MAX_RHS));
+        OVL_TRY(dev_alloc(c, (void **)&c->coef_dev, sizeof(double) * nev));
         c->proj_cap = nev;
     }
     const size_t vb = c->n() * sizeof(double2);  // one canonical complex128 vector
@@ -278,16 +384,7 @@ int ovl_cg_multi(ovl_ctx *c, int nrhs, double mu, const void *b, void *x, double
     if (!b || !x || b == x || !iters_out || !relres_out || maxiter < 0) return fail(c, OVL_EINVAL, "bad ovl_cg_multi arguments");
     if (nrhs < 1 || nrhs > OVL_MAX_RHS) return fail(c, OVL_EINVAL, "nrhs must be in 1..%d", OVL_MAX_RHS);
     if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
-    if (nrhs > c->multi_cap) {
-        OVL_CUDA(c, cudaStreamSynchronize(c->st));
-        if (c->multi_in) cudaFree(c->multi_in);
-        if (c->multi_out) cudaFree(c->multi_out);
-        c->multi_in = c->multi_out = nullptr;
-        c->multi_cap = 0;
-        OVL_TRY(dev_alloc(c, &c->multi_in, c->field_bytes() * nrhs));
-        OVL_TRY(dev_alloc(c, &c->multi_out, c->field_bytes() * nrhs));
-        c->multi_cap = nrhs;
-    }
+    OVL_TRY(ensure_multi_staging(c, nrhs));
     const size_t cb = c->canon_bytes(), fb = c->field_bytes();
     for (int r = 0; r < nrhs; ++r) OVL_TRY(import_any(c, (const char *)b + r * cb, (char *)c->multi_in + r * fb));
     int rc = DISPATCH(c, cg_native, c, mu, c->multi_in, c->multi_out, tol, maxiter, iters_out, relres_out, nrhs);
@@ -358,16 +455,7 @@ int ovl_overlap_multi(ovl_ctx *c, int nrhs, double mu, int dagger, const void *p
     if (!c) return OVL_EINVAL;
     if (!psi || !out || psi == out) return fail(c, OVL_EINVAL, "null or aliased spinor pointers");
     if (nrhs < 1 || nrhs > OVL_MAX_RHS) return fail(c, OVL_EINVAL, "nrhs must be in 1..%d", OVL_MAX_RHS);
-    if (nrhs > c->multi_cap) {
-        OVL_CUDA(c, cudaStreamSynchronize(c->st));
-        if (c->multi_in) cudaFree(c->multi_in);
-        if (c->multi_out) cudaFree(c->multi_out);
-        c->multi_in = c->multi_out = nullptr;
-        c->multi_cap = 0;
-        OVL_TRY(dev_alloc(c, &c->multi_in, c->field_bytes() * nrhs));
-        OVL_TRY(dev_alloc(c, &c->multi_out, c->field_bytes() * nrhs));
-        c->multi_cap = nrhs;
-    }
+    OVL_TRY(ensure_multi_staging(c, nrhs));
     const size_t cb = c->canon_bytes(), fb = c->field_bytes();
     for (int r = 0; r < nrhs; ++r)
         OVL_TRY(import_any(c, (const char *)psi + r * cb, (char *)c->multi_in + r * fb));

@@ -62,81 +62,122 @@ __device__ __forceinline__ double block_sum(double v, double *sm) {
     return r;
 }
 
-// ---------------------------------------------------------------- a5: c_i = phi_i^dag psi, i < nev
-// grid = (nblk, 1); block b owns the elements [b*CH, (b+1)*CH) of the flat 12V-complex field for ALL i:
-// psi chunk held in registers, every phi_i streamed once.  partial[i*nblk + b] (complex fp64).
-constexpr int PROJ_EPT = 4;  // elements per thread
+// ---------------------------------------------------------------- a5: c_{r,i} = phi_i^dag psi_r, i < nev, r < nrhs
+// grid = (nblk, ceil(nrhs / DEFL_RB)); block b owns the elements [b*CH, (b+1)*CH) of the flat 12V-complex field for ALL i
+// and for a group of DEFL_RB right-hand sides: the psi chunks of the group stay in registers and every phi_i is streamed
+// ONCE per group (not once per right-hand side).  partial[((r * nev) + i) * nblk + b]  (complex fp64).
+// The reduction tree per (r, i) -- thread-serial over the chunk, warp shuffle, warps 0..7 in order -- does not depend on
+// the group size, so a right-hand side gets bit-identical coefficients whether it is projected alone or in a batch.
+constexpr int PROJ_EPT = 4;   // elements per thread
+constexpr int DEFL_RB = 4;    // right-hand sides per group
 template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS)
-k_project(size_t n, int nev, const cx<T> *__restrict__ phi, const cx<T> *__restrict__ psi, double2 *__restrict__ partial) {
-    __shared__ double sm[2 * (BLAS_THREADS / 32)];
+k_project(size_t n, int nev, int nrhs, const cx<T> *__restrict__ phi, const cx<T> *__restrict__ psi, double2 *__restrict__ partial) {
+    __shared__ double sm[2][BLAS_THREADS / 32][2 * DEFL_RB];
     const size_t base = (size_t)blockIdx.x * (BLAS_THREADS * PROJ_EPT) + threadIdx.x;
-    cx<T> p[PROJ_EPT];
+    const int r0 = blockIdx.y * DEFL_RB;
+    const int nr = min(DEFL_RB, nrhs - r0);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    cx<T> p[DEFL_RB][PROJ_EPT];
 #pragma unroll
-    for (int j = 0; j < PROJ_EPT; ++j) {
-        const size_t e = base + (size_t)j * BLAS_THREADS;
-        p[j] = e < n ? psi[e] : mk<T>(0, 0);
-    }
-    for (int i = 0; i < nev; ++i) {
-        const cx<T> *ph = phi + (size_t)i * n;
-        double re = 0, im = 0;
+    for (int r = 0; r < DEFL_RB; ++r)
 #pragma unroll
         for (int j = 0; j < PROJ_EPT; ++j) {
             const size_t e = base + (size_t)j * BLAS_THREADS;
-            if (e < n) {
-                const cx<T> f = ldg(ph + e);
-                re += (double)f.x * (double)p[j].x + (double)f.y * (double)p[j].y;
-                im += (double)f.x * (double)p[j].y - (double)f.y * (double)p[j].x;
+            p[r][j] = (r < nr && e < n) ? psi[(size_t)(r0 + r) * n + e] : mk<T>(0, 0);
+        }
+    for (int i = 0; i < nev; ++i) {
+        const cx<T> *ph = phi + (size_t)i * n;
+        cx<T> f[PROJ_EPT];
+#pragma unroll
+        for (int j = 0; j < PROJ_EPT; ++j) {
+            const size_t e = base + (size_t)j * BLAS_THREADS;
+            f[j] = e < n ? ldg(ph + e) : mk<T>(0, 0);
+        }
+        double (*buf)[2 * DEFL_RB] = sm[i & 1];
+#pragma unroll
+        for (int r = 0; r < DEFL_RB; ++r) {
+            if (r < nr) {
+                double re = 0, im = 0;
+#pragma unroll
+                for (int j = 0; j < PROJ_EPT; ++j) {
+                    if (base + (size_t)j * BLAS_THREADS < n) {
+                        re += (double)f[j].x * (double)p[r][j].x + (double)f[j].y * (double)p[r][j].y;
+                        im += (double)f[j].x * (double)p[r][j].y - (double)f[j].y * (double)p[r][j].x;
+                    }
+                }
+                re = warp_sum(re);
+                im = warp_sum(im);
+                if (l == 0) { buf[w][2 * r] = re; buf[w][2 * r + 1] = im; }
             }
         }
-        const double r0 = block_sum(re, sm);
-        const double r1 = block_sum(im, sm + BLAS_THREADS / 32);
-        if (threadIdx.x == 0) partial[(size_t)i * gridDim.x + blockIdx.x] = make_double2(r0, r1);
+        __syncthreads();  // (the other half of sm is rewritten only after the next barrier)
+        if (threadIdx.x < nr) {
+            double re = 0, im = 0;
+            for (int q = 0; q < BLAS_THREADS / 32; ++q) { re += buf[q][2 * threadIdx.x]; im += buf[q][2 * threadIdx.x + 1]; }
+            partial[((size_t)(r0 + threadIdx.x) * nev + i) * gridDim.x + blockIdx.x] = make_double2(re, im);
+        }
     }
 }
-// second stage: one block per i; w_i = coef_i * sum_b partial[i][b]   (a6: coef_i = sign(lambda_i) - p(lambda^_i))
+// second stage: one block per (i, r); w[r * wstride + i] = coef_i * sum_b partial[r][i][b]   (a6: coef_i = sign(lambda_i) - p(lambda^_i))
 __global__ void __launch_bounds__(BLAS_THREADS)
-k_project_final(int nblk, const double2 *__restrict__ partial, const double *__restrict__ coef, double2 *__restrict__ w) {
+k_project_final(int nblk, int nev, int wstride, const double2 *__restrict__ partial, const double *__restrict__ coef, double2 *__restrict__ w) {
     __shared__ double sm[2 * (BLAS_THREADS / 32)];
-    const int i = blockIdx.x;
+    const int i = blockIdx.x, r = blockIdx.y;
+    const double2 *p = partial + ((size_t)r * nev + i) * nblk;
     double re = 0, im = 0;
     for (int b = threadIdx.x; b < nblk; b += blockDim.x) {
-        const double2 v = partial[(size_t)i * nblk + b];
+        const double2 v = p[b];
         re += v.x; im += v.y;
     }
-    const double r0 = block_sum(re, sm);
-    const double r1 = block_sum(im, sm + BLAS_THREADS / 32);
-    if (threadIdx.x == 0) w[i] = make_double2(coef[i] * r0, coef[i] * r1);
+    const double q0 = block_sum(re, sm);
+    const double q1 = block_sum(im, sm + BLAS_THREADS / 32);
+    if (threadIdx.x == 0) w[(size_t)r * wstride + i] = make_double2(coef[i] * q0, coef[i] * q1);
 }
 
-// ---------------------------------------------------------------- a7 + a8: s = acc + sum_i w_i phi_i;  out = a psi + b [gamma5] s
-// flat element e = k*V + s: gamma5 is -1 for e >= 6V (planes of spin 2,3).
+// ---------------------------------------------------------------- a7 + a8: s_r = acc_r + sum_i w_{r,i} phi_i;  out_r = a psi_r + b [gamma5] s_r
+// flat element e = k*V + s: gamma5 is -1 for e >= 6V (planes of spin 2,3).  grid.y = groups of DEFL_RB right-hand sides:
+// every phi_i[e] is loaded once per group.  The deflation sum is carried in fp64 and added to the polynomial part once.
 template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS)
-k_deflate_assemble(size_t n, size_t n_upper, int nev, const cx<T> *__restrict__ phi, const double2 *__restrict__ w,
+k_deflate_assemble(size_t n, size_t n_upper, int nev, int nrhs, int wstride, const cx<T> *__restrict__ phi, const double2 *__restrict__ w,
                    const cx<T> *__restrict__ psi, const cx<T> *__restrict__ acc, T a, T b, int g5, cx<T> *__restrict__ out) {
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n) return;
-    const cx<T> s0 = acc[e];
-    // the deflation sum is carried in fp64 and added to the polynomial part once
-    double re = 0, im = 0;
+    const int r0 = blockIdx.y * DEFL_RB;
+    const int nr = min(DEFL_RB, nrhs - r0);
+    double re[DEFL_RB], im[DEFL_RB];
+#pragma unroll
+    for (int r = 0; r < DEFL_RB; ++r) re[r] = im[r] = 0.0;
     for (int i = 0; i < nev; ++i) {
         const cx<T> f = ldg(phi + (size_t)i * n + e);
-        const double2 wi = w[i];
-        re += wi.x * (double)f.x - wi.y * (double)f.y;
-        im += wi.x * (double)f.y + wi.y * (double)f.x;
+#pragma unroll
+        for (int r = 0; r < DEFL_RB; ++r) {
+            if (r < nr) {
+                const double2 wi = w[(size_t)(r0 + r) * wstride + i];
+                re[r] += wi.x * (double)f.x - wi.y * (double)f.y;
+                im[r] += wi.x * (double)f.y + wi.y * (double)f.x;
+            }
+        }
     }
-    T sx = (T)((double)s0.x + re), sy = (T)((double)s0.y + im);
-    if (g5 && e >= n_upper) { sx = -sx; sy = -sy; }
-    cx<T> r;
-    if (a != T(0)) {
-        const cx<T> p = psi[e];
-        r.x = fma(a, p.x, b * sx);
-        r.y = fma(a, p.y, b * sy);
-    } else {
-        r.x = b * sx; r.y = b * sy;
+#pragma unroll
+    for (int r = 0; r < DEFL_RB; ++r) {
+        if (r < nr) {
+            const size_t o = (size_t)(r0 + r) * n + e;
+            const cx<T> s0 = acc[o];
+            T sx = (T)((double)s0.x + re[r]), sy = (T)((double)s0.y + im[r]);
+            if (g5 && e >= n_upper) { sx = -sx; sy = -sy; }
+            cx<T> q;
+            if (a != T(0)) {
+                const cx<T> pp = psi[o];
+                q.x = fma(a, pp.x, b * sx);
+                q.y = fma(a, pp.y, b * sy);
+            } else {
+                q.x = b * sx; q.y = b * sy;
+            }
+            out[o] = q;
+        }
     }
-    out[e] = r;
 }
 
 // out = gamma5 in (only used to form the input of sign() in D^dag)
@@ -144,6 +185,7 @@ template <typename T>
 __global__ void k_gamma5(size_t n, size_t n_upper, const cx<T> *__restrict__ in, cx<T> *__restrict__ out) {
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n) return;
+    in += blockIdx.y * n; out += blockIdx.y * n;  // blockIdx.y = right-hand side
     cx<T> v = in[e];
     if (e >= n_upper) { v.x = -v.x; v.y = -v.y; }
     out[e] = v;

@@ -36,8 +36,9 @@ struct ovl_ctx {
     void *stage_in = nullptr, *stage_out = nullptr;  // canonical staging for host pointers (12V complex128 each)
     double2 *proj_partial = nullptr, *w_dev = nullptr;
     double *coef_dev = nullptr;
-    int proj_nblk = 0, proj_cap = 0;
-    double *red_partial = nullptr, *sc_dev = nullptr, *sc_host = nullptr;
+    int proj_nblk = 0, proj_cap = 0, proj_rhs = 0;  // blocks of the projection grid; eigenvector / right-hand-side capacity of its scratch
+    double *red_partial = nullptr, *sc_dev = nullptr, *sc_host = nullptr;  // sc_host: two pinned slots of SC_N * OVL_MAX_RHS
+    cudaEvent_t cg_ev[2] = {nullptr, nullptr};                             // read-back events of the pipelined CG check
     int red_nblk = 0;
 
     // CUDA graphs of the polynomial loop (one per source field), replayed instead of re-issuing norders launches
@@ -59,6 +60,16 @@ struct ovl_ctx {
     long long prof_count = 0;         // profiled loops since ovl_set_profiling(on)
     int last_poly_launches = 0;
     long long launches = 0;
+
+    // memory: either one caller-owned workspace (ovl_create_ws: everything below is carved from it at create time and
+    // nothing is allocated afterwards) or library-owned allocations (ovl_create: one cudaMalloc for the base set, more
+    // only when a capacity grows: eigenvector store, multi-rhs workspaces, eigensolver block)
+    struct Arena { char *base = nullptr; size_t size = 0, off = 0; } arena;
+    bool ws_mode = false;            // caller-owned workspace: never cudaMalloc / cudaFree
+    std::vector<void *> owned;       // library-owned device allocations (freed by ovl_destroy)
+    int max_nev = 0, max_rhs = 1, eig_cap = 0;   // capacities of a caller-owned workspace
+    void *eig_ws = nullptr;          // eigensolver block inside a caller-owned workspace
+    size_t eig_ws_bytes = 0;
 
     char err[256] = {0};
 
@@ -108,10 +119,34 @@ inline bool is_device_ptr(const void *p) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
+constexpr size_t WS_ALIGN = 256;
+inline size_t ws_round(size_t b) { return (b + WS_ALIGN - 1) / WS_ALIGN * WS_ALIGN; }
+
+// Device memory for the context: carved from the arena while it has room; otherwise cudaMalloc -- unless the context
+// lives in a caller-owned workspace, where running out is an error (the capacity was fixed by ovl_workspace_bytes).
 inline int dev_alloc(ovl_ctx *c, void **p, size_t bytes) {
     if (*p) return OVL_OK;
-    OVL_CUDA(c, cudaMalloc(p, bytes ? bytes : 16));
+    const size_t b = ws_round(bytes ? bytes : 16);
+    if (c->arena.base && c->arena.off + b <= c->arena.size) {
+        *p = c->arena.base + c->arena.off;
+        c->arena.off += b;
+        return OVL_OK;
+    }
+    if (c->ws_mode) return fail(c, OVL_ENOMEM, "the caller-owned workspace is exhausted (%zu more bytes needed)", b);
+    OVL_CUDA(c, cudaMalloc(p, b));
+    c->owned.push_back(*p);
     return OVL_OK;
+}
+// give a buffer back: only library-owned allocations are freed (arena memory lives until ovl_destroy)
+inline void dev_release(ovl_ctx *c, void **p) {
+    if (!*p) return;
+    for (size_t i = 0; i < c->owned.size(); ++i)
+        if (c->owned[i] == *p) {
+            cudaFree(*p);
+            c->owned.erase(c->owned.begin() + i);
+            break;
+        }
+    *p = nullptr;
 }
 
 inline int grid_for(size_t n, int threads, int cap = 148 * 16) {

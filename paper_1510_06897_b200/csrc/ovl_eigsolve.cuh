@@ -21,17 +21,65 @@
 
 namespace ovl {
 
+// The work block of one ovl_lowest_eigenpairs call for `cap` = max(block, 2 nev) vectors: one contiguous device region,
+// either inside the caller-owned workspace (eig_block of ovl_workspace_bytes) or one cudaMalloc released on return.
 struct EigWork {
     double2 *V = nullptr, *W = nullptr, *Z = nullptr, *R = nullptr, *Q = nullptr, *gram_partial = nullptr, *C = nullptr, *X = nullptr;
     double *partial = nullptr, *small = nullptr;  // small: theta / scales / norms, cap doubles each (3 cap)
     int cap = 0;                                  // vectors per work block
+    void *owned = nullptr;
     ~EigWork() {
-        void *p[] = {V, W, Z, R, Q, gram_partial, C, X, partial, small};
-        for (void *q : p)
-            if (q) cudaFree(q);
+        if (owned) cudaFree(owned);
         cudaGetLastError();
     }
 };
+template <typename F> inline void eig_ws_visit(size_t V, int cap, F f) {
+    const size_t n = 12 * V, fb = n * sizeof(double2);
+    const size_t nblk_g = (n + BLAS_THREADS * GRAM_EPT - 1) / (BLAS_THREADS * GRAM_EPT), nchunk_g = (cap + GRAM_J - 1) / GRAM_J;
+    const size_t nb = grid_for(n, BLAS_THREADS * 4, 148 * 8);
+    f(0, fb * cap); f(1, fb * cap); f(2, fb * cap); f(3, fb * cap); f(4, fb * cap);            // V W Z R Q
+    f(5, sizeof(double2) * (size_t)cap * GRAM_J * nblk_g * (BLAS_THREADS / 32));               // gram_partial
+    f(6, sizeof(double2) * nchunk_g * cap * GRAM_J);                                            // C
+    f(7, sizeof(double2) * (size_t)cap * cap);                                                  // X
+    f(8, sizeof(double) * nb * cap);                                                            // partial
+    f(9, sizeof(double) * 3 * cap);                                                             // small
+}
+inline size_t eig_ws_total(size_t V, int cap) {
+    size_t t = 0;
+    eig_ws_visit(V, cap, [&](int, size_t b) { t += ws_round(b); });
+    return t;
+}
+inline int eig_ws_setup(ovl_ctx *c, EigWork &w, int cap) {
+    const size_t need = eig_ws_total(c->g.V, cap);
+    char *base = nullptr;
+    if (c->ws_mode) {
+        if (cap > c->eig_cap || need > c->eig_ws_bytes)
+            return fail(c, OVL_EINVAL, "the eigensolver needs a work block of %d vectors; the workspace was sized for eig_block = %d", cap, c->eig_cap);
+        base = (char *)c->eig_ws;
+    } else {
+        OVL_CUDA(c, cudaMalloc(&w.owned, need));
+        base = (char *)w.owned;
+    }
+    w.cap = cap;
+    size_t off = 0;
+    eig_ws_visit(c->g.V, cap, [&](int id, size_t b) {
+        void *p = base + off;
+        off += ws_round(b);
+        switch (id) {
+            case 0: w.V = (double2 *)p; break;
+            case 1: w.W = (double2 *)p; break;
+            case 2: w.Z = (double2 *)p; break;
+            case 3: w.R = (double2 *)p; break;
+            case 4: w.Q = (double2 *)p; break;
+            case 5: w.gram_partial = (double2 *)p; break;
+            case 6: w.C = (double2 *)p; break;
+            case 7: w.X = (double2 *)p; break;
+            case 8: w.partial = (double *)p; break;
+            case 9: w.small = (double *)p; break;
+        }
+    });
+    return OVL_OK;
+}
 
 // C (host, m x m row-major) = A^dag B for the m-vector blocks A, B
 inline int eig_gram(ovl_ctx *c, EigWork &w, int m, const double2 *A, const double2 *B, dense::mat &out) {
@@ -199,24 +247,11 @@ inline int eig_lowest(ovl_ctx *c, int nev, double tol, int max_cycles, int degre
     if ((size_t)m > n) return fail(c, OVL_EINVAL, "block size %d exceeds the dimension of the space", m);
     if (degree < 1) degree = 1;
     const int cap = std::max(m, 2 * nev);  // vectors per work block
-    const int chunk = std::min(m, (int)OVL_MAX_RHS);
+    const int chunk = std::min(m, c->ws_mode ? c->max_rhs : (int)OVL_MAX_RHS);  // vectors per filter pass (recurrence workspace)
     OVL_TRY(ensure_work(c, chunk));
     EigWork w;
-    w.cap = cap;
-    const size_t bb = c->field_bytes() * cap;
-    const int nblk_g = (int)((n + BLAS_THREADS * GRAM_EPT - 1) / (BLAS_THREADS * GRAM_EPT));
-    const int nchunk_g = (cap + GRAM_J - 1) / GRAM_J;
+    OVL_TRY(eig_ws_setup(c, w, cap));
     const int nb = c->red_nblk;
-    OVL_CUDA(c, cudaMalloc((void **)&w.V, bb));
-    OVL_CUDA(c, cudaMalloc((void **)&w.W, bb));
-    OVL_CUDA(c, cudaMalloc((void **)&w.Z, bb));
-    OVL_CUDA(c, cudaMalloc((void **)&w.R, bb));
-    OVL_CUDA(c, cudaMalloc((void **)&w.Q, c->field_bytes() * 2 * nev));
-    OVL_CUDA(c, cudaMalloc((void **)&w.gram_partial, sizeof(double2) * (size_t)cap * GRAM_J * nblk_g * (BLAS_THREADS / 32)));
-    OVL_CUDA(c, cudaMalloc((void **)&w.C, sizeof(double2) * (size_t)nchunk_g * cap * GRAM_J));
-    OVL_CUDA(c, cudaMalloc((void **)&w.X, sizeof(double2) * (size_t)cap * cap));
-    OVL_CUDA(c, cudaMalloc((void **)&w.partial, sizeof(double) * (size_t)nb * cap));
-    OVL_CUDA(c, cudaMalloc((void **)&w.small, sizeof(double) * 3 * cap));
     double *scale_d = w.small + cap, *norm_d = w.small + 2 * cap;
 
     for (int j = 0; j < m; ++j) {

@@ -195,21 +195,23 @@ inline int refresh_coef(ovl_ctx *c) {
     return OVL_OK;
 }
 
-// work vectors of the recurrence (t_A, t_B, acc, gamma5 psi) for `nrhs` right-hand sides; grown on demand
+// work vectors of the recurrence (t_A, t_B, acc, gamma5 psi) for `nrhs` right-hand sides; grown on demand when the library
+// owns the memory, fixed at max_rhs in a caller-owned workspace
 inline int ensure_work(ovl_ctx *c, int nrhs) {
     if (nrhs <= c->work_nrhs) return OVL_OK;
+    if (c->ws_mode) return fail(c, OVL_EINVAL, "%d right-hand sides exceed the workspace capacity max_rhs = %d", nrhs, c->max_rhs);
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     void **bufs[] = {&c->tA, &c->tB, &c->acc, &c->g5b};
     void *fresh[4] = {nullptr, nullptr, nullptr, nullptr};
     for (int i = 0; i < 4; ++i) {
         const int rc = dev_alloc(c, &fresh[i], c->field_bytes() * nrhs);
         if (rc != OVL_OK) {  // keep the old (smaller) workspace usable
-            for (int j = 0; j < i; ++j) cudaFree(fresh[j]);
+            for (int j = 0; j < i; ++j) dev_release(c, &fresh[j]);
             return rc;
         }
     }
     for (int i = 0; i < 4; ++i) {
-        if (*bufs[i]) cudaFree(*bufs[i]);
+        dev_release(c, bufs[i]);
         *bufs[i] = fresh[i];
     }
     c->work_nrhs = nrhs;
@@ -217,37 +219,48 @@ inline int ensure_work(ovl_ctx *c, int nrhs) {
     return OVL_OK;
 }
 
+// scratch of the projection for nrhs right-hand sides (library-owned contexts grow it; a workspace holds max_rhs)
+inline int ensure_proj(ovl_ctx *c, int nrhs) {
+    if (nrhs <= c->proj_rhs) return OVL_OK;
+    if (c->ws_mode) return fail(c, OVL_EINVAL, "%d right-hand sides exceed the workspace capacity max_rhs = %d", nrhs, c->max_rhs);
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    dev_release(c, (void **)&c->proj_partial);
+    c->proj_rhs = 0;
+    OVL_TRY(dev_alloc(c, (void **)&c->proj_partial, sizeof(double2) * (size_t)c->proj_nblk * c->proj_cap * nrhs));
+    c->proj_rhs = nrhs;
+    return OVL_OK;
+}
+
 // out_r = a*in_r + b*[gamma5]( sign(K) src_r ) for r < nrhs consecutive native fields;  src = in (dagger = 0) or gamma5 in
 // (dagger = 1, gamma5 not applied on the way out).  ovl_sign uses a = 0, b = 1, g5out = 0.  The polynomial loop handles
-// all right-hand sides in every launch (links amortised); the deflation passes run per right-hand side.
+// all right-hand sides in every launch (links amortised); the two deflation passes read every phi_i once per group of
+// DEFL_RB right-hand sides.
 template <typename T> int sign_combine_native(ovl_ctx *c, int nrhs, double a, double b, int dagger, int g5out, const void *in, void *out) {
     if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
     OVL_TRY(ensure_work(c, nrhs));
     const size_t n = c->n(), n_upper = (size_t)6 * c->g.V;
     const void *src = in;
     if (dagger) {
-        for (int r = 0; r < nrhs; ++r) {
-            k_gamma5<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(n, n_upper, (const cx<T> *)in + r * n, (cx<T> *)c->g5b + r * n);
-            OVL_LAUNCH_CHECK(c);
-        }
+        k_gamma5<T><<<dim3(grid_for(n, BLAS_THREADS, 1 << 30), nrhs), BLAS_THREADS, 0, c->st>>>(n, n_upper, (const cx<T> *)in, (cx<T> *)c->g5b);
+        OVL_LAUNCH_CHECK(c);
         src = c->g5b;
     }
+    const int ngrp = (nrhs + DEFL_RB - 1) / DEFL_RB;
     if (c->nev > 0) {
         OVL_TRY(refresh_coef(c));
-        for (int r = 0; r < nrhs; ++r) {
-            k_project<T><<<c->proj_nblk, BLAS_THREADS, 0, c->st>>>(n, c->nev, (const cx<T> *)c->phi, (const cx<T> *)src + r * n, c->proj_partial);
-            OVL_LAUNCH_CHECK(c);
-            k_project_final<<<c->nev, BLAS_THREADS, 0, c->st>>>(c->proj_nblk, c->proj_partial, c->coef_dev, c->w_dev + (size_t)r * c->proj_cap);
-            OVL_LAUNCH_CHECK(c);
-        }
-    }
-    OVL_TRY(cheb_native<T>(c, src, nrhs));
-    for (int r = 0; r < nrhs; ++r) {
-        k_deflate_assemble<T><<<grid_for(n, BLAS_THREADS, 1 << 30), BLAS_THREADS, 0, c->st>>>(
-            n, n_upper, c->nev, (const cx<T> *)c->phi, c->w_dev + (size_t)r * c->proj_cap, (const cx<T> *)in + r * n,
-            (const cx<T> *)c->acc + r * n, (T)a, (T)b, g5out, (cx<T> *)out + r * n);
+        OVL_TRY(ensure_proj(c, nrhs));
+        // phi_i is streamed once per group of DEFL_RB right-hand sides (projection) ...
+        k_project<T><<<dim3(c->proj_nblk, ngrp), BLAS_THREADS, 0, c->st>>>(n, c->nev, nrhs, (const cx<T> *)c->phi, (const cx<T> *)src, c->proj_partial);
+        OVL_LAUNCH_CHECK(c);
+        k_project_final<<<dim3(c->nev, nrhs), BLAS_THREADS, 0, c->st>>>(c->proj_nblk, c->nev, c->proj_cap, c->proj_partial, c->coef_dev, c->w_dev);
         OVL_LAUNCH_CHECK(c);
     }
+    OVL_TRY(cheb_native<T>(c, src, nrhs));
+    // ... and once more per group in the update + assembly pass
+    k_deflate_assemble<T><<<dim3(grid_for(n, BLAS_THREADS, 1 << 30), ngrp), BLAS_THREADS, 0, c->st>>>(
+        n, n_upper, c->nev, nrhs, c->proj_cap > 0 ? c->proj_cap : 1, (const cx<T> *)c->phi, c->w_dev, (const cx<T> *)in, (const cx<T> *)c->acc, (T)a,
+        (T)b, g5out, (cx<T> *)out);
+    OVL_LAUNCH_CHECK(c);
     return OVL_OK;
 }
 
@@ -266,19 +279,17 @@ template <typename T> int reduce_redot(ovl_ctx *c, const void *x, const void *y,
     OVL_LAUNCH_CHECK(c);
     return OVL_OK;
 }
-inline int fetch_scalars(ovl_ctx *c, int nrhs) {
+inline int fetch_scalars(ovl_ctx *c, int nrhs) {  // synchronous read-out into slot 0 (start-up and final residual only)
     OVL_CUDA(c, cudaMemcpyAsync(c->sc_host, c->sc_dev, sizeof(double) * SC_N * nrhs, cudaMemcpyDeviceToHost, c->st));
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     return OVL_OK;
 }
 inline int ensure_cg(ovl_ctx *c, int nrhs) {
     if (nrhs <= c->cg_nrhs) return OVL_OK;
+    if (c->ws_mode) return fail(c, OVL_EINVAL, "%d systems exceed the workspace capacity max_rhs = %d", nrhs, c->max_rhs);
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     void **bufs[] = {&c->cg_r, &c->cg_p, &c->cg_q, &c->cg_Ap};
-    for (void **b : bufs) {
-        if (*b) cudaFree(*b);
-        *b = nullptr;
-    }
+    for (void **b : bufs) dev_release(c, b);
     c->cg_nrhs = 0;
     for (void **b : bufs) OVL_TRY(dev_alloc(c, b, c->field_bytes() * nrhs));
     c->cg_nrhs = nrhs;
@@ -304,30 +315,43 @@ int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int
         conv[r] = tol > 0 && rr[r] <= tol2 * bb[r];  // b = 0
         nconv += conv[r];
     }
-    int it = 0;
     const dim3 gridv(grid_for(n, BLAS_THREADS), nrhs), gridr(c->red_nblk, nrhs);
-    while (it < maxiter && nconv < nrhs) {
+    // The host never stalls the device between iterations: iteration `it` is enqueued BEFORE the convergence scalars of
+    // iteration it-1 are read (asynchronous copy into one of two pinned slots + an event).  A system that has reached the
+    // tolerance is frozen on the device in the same kernel that forms beta (alpha = beta = 0 from then on: x and r stop
+    // changing), so the one iteration that may run past convergence leaves the solution bit-identical.
+    int enq = 0, seen = 0;
+    auto check = [&](int j) -> int {  // consume the scalars of iteration j (0-based)
+        OVL_CUDA(c, cudaEventSynchronize(c->cg_ev[j & 1]));
+        const double *h = c->sc_host + (size_t)(j & 1) * SC_N * OVL_MAX_RHS;
+        for (int r = 0; r < nrhs; ++r) {
+            if (conv[r]) continue;
+            rr[r] = h[r * SC_N + SC_RR];
+            iters[r] = j + 1;
+            if (!(rr[r] == rr[r])) return fail(c, OVL_ECUDA, "CG broke down (NaN residual) at iteration %d, system %d", j + 1, r);
+            if (tol > 0 && rr[r] <= tol2 * bb[r]) { conv[r] = true; ++nconv; }  // same test as the device-side freeze
+        }
+        return OVL_OK;
+    };
+    while (enq < maxiter && nconv < nrhs) {
         OVL_TRY(overlap_native<T>(c, mu, 0, c->cg_p, c->cg_q, nrhs));
         OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap, nrhs));
         OVL_TRY(reduce_redot<T>(c, c->cg_p, c->cg_Ap, 1, nrhs));  // alpha = rr / Re(p^dag A p)
         k_cg_update<T><<<gridr, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_p, (const cx<T> *)c->cg_Ap,
                                                         (cx<T> *)x_n, (cx<T> *)c->cg_r, c->red_partial);
         OVL_LAUNCH_CHECK(c);
-        // beta, rr; with several systems the converged ones are frozen on the device (a single system just stops)
-        k_cg_scalars<<<nrhs, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, 2, nrhs > 1 ? tol2 : 0.0);
+        k_cg_scalars<<<nrhs, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, c->sc_dev, 2, tol2);  // beta, rr, freeze
         OVL_LAUNCH_CHECK(c);
         k_xpay<T><<<gridv, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_r, (cx<T> *)c->cg_p);
         OVL_LAUNCH_CHECK(c);
-        OVL_TRY(fetch_scalars(c, nrhs));  // the convergence scalars are the only host round trip per iteration
-        ++it;
-        for (int r = 0; r < nrhs; ++r) {
-            if (conv[r]) continue;
-            rr[r] = c->sc_host[r * SC_N + SC_RR];
-            iters[r] = it;
-            if (!(rr[r] == rr[r])) return fail(c, OVL_ECUDA, "CG broke down (NaN residual) at iteration %d, system %d", it, r);
-            if (tol > 0 && rr[r] <= tol2 * bb[r]) { conv[r] = true; ++nconv; }  // same test as the device-side freeze
-        }
+        OVL_CUDA(c, cudaMemcpyAsync(c->sc_host + (size_t)(enq & 1) * SC_N * OVL_MAX_RHS, c->sc_dev, sizeof(double) * SC_N * nrhs,
+                                    cudaMemcpyDeviceToHost, c->st));
+        OVL_CUDA(c, cudaEventRecord(c->cg_ev[enq & 1], c->st));
+        ++enq;
+        if (enq - seen == 2) OVL_TRY(check(seen++));  // one iteration behind the device
     }
+    while (seen < enq && nconv < nrhs) OVL_TRY(check(seen++));
+    const int it = enq;
     // true residuals ||b - A x|| / ||b||
     OVL_TRY(overlap_native<T>(c, mu, 0, x_n, c->cg_q, nrhs));
     OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap, nrhs));

@@ -64,18 +64,11 @@ __device__ __forceinline__ void load_link(cx<T> (&u)[3][3], const cx<T> *__restr
     }
 }
 
-// One hop: MU direction, FWD = 1: (1 - gamma_mu) U_mu(x) in(x+mu);  FWD = 0: (1 + gamma_mu) U_mu(x-mu)^dag in(x-mu).
-// sn = neighbour site, su = site that owns the link, bs = boundary phase (+1 / -1).
-template <typename T, int RECON, int MU, int FWD>
-__device__ __forceinline__ void hop_dir(cx<T> (&hop)[12], const cx<T> *__restrict__ in, const cx<T> *__restrict__ U,
-                                        int V, int sn, int su, T bs) {
-    constexpr int NROW = RECON == 18 ? 3 : 2;
-    cx<T> p[12];
-#pragma unroll
-    for (int k = 0; k < 12; ++k) p[k] = ldg(in + (size_t)k * V + sn);
-    cx<T> u[3][3];
-    load_link<T, RECON>(u, U + (size_t)MU * NROW * 3 * V, V, su);
-
+// The arithmetic of one hop given the neighbour spinor p and the link u (already in registers): spin projection to a half
+// spinor, 3x3 colour multiply (U for FWD = 1, U^dag for FWD = 0), reconstruction into the 12 accumulators.
+// MU direction, FWD = 1: (1 - gamma_mu) U_mu(x) in(x+mu);  FWD = 0: (1 + gamma_mu) U_mu(x-mu)^dag in(x-mu); bs = boundary phase.
+template <typename T, int MU, int FWD>
+__device__ __forceinline__ void hop_math(cx<T> (&hop)[12], const cx<T> (&p)[12], const cx<T> (&u)[3][3], T bs) {
     cx<T> h0[3], h1[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -93,8 +86,10 @@ __device__ __forceinline__ void hop_dir(cx<T> (&hop)[12], const cx<T> *__restric
             h0[c] = FWD ? csub(p0, p2) : cadd(p0, p2);
             h1[c] = FWD ? csub(p1, p3) : cadd(p1, p3);
         }
-        h0[c].x *= bs; h0[c].y *= bs;
-        h1[c].x *= bs; h1[c].y *= bs;
+        if (MU == 3) {  // only the t hops can cross the antiperiodic boundary (bs = +-1; elsewhere it is exactly 1)
+            h0[c].x *= bs; h0[c].y *= bs;
+            h1[c].x *= bs; h1[c].y *= bs;
+        }
     }
     cx<T> g0[3], g1[3];
 #pragma unroll
@@ -131,6 +126,19 @@ __device__ __forceinline__ void hop_dir(cx<T> (&hop)[12], const cx<T> *__restric
             hop[9 + c] = FWD ? csub(hop[9 + c], g1[c]) : cadd(hop[9 + c], g1[c]);
         }
     }
+}
+
+// One hop with both operands loaded from global memory: sn = neighbour site, su = site that owns the link.
+template <typename T, int RECON, int MU, int FWD>
+__device__ __forceinline__ void hop_dir(cx<T> (&hop)[12], const cx<T> *__restrict__ in, const cx<T> *__restrict__ U,
+                                        int V, int sn, int su, T bs) {
+    constexpr int NROW = RECON == 18 ? 3 : 2;
+    cx<T> p[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) p[k] = ldg(in + (size_t)k * V + sn);
+    cx<T> u[3][3];
+    load_link<T, RECON>(u, U + (size_t)MU * NROW * 3 * V, V, su);
+    hop_math<T, MU, FWD>(hop, p, u, bs);
 }
 
 template <typename T, int RECON, int MU>

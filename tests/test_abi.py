@@ -65,7 +65,21 @@ def test_host_side_argument_checks_without_gpu(lib_path):
     assert lib.ovl_device_bytes(dims, 7, B.OVL_RECON18, 0) == 0
     bad = (ctypes.c_int * 4)(4, 4, 1, 4)
     assert lib.ovl_device_bytes(bad, B.OVL_F64, B.OVL_RECON18, 0) == 0
+    # the workspace plan: monotone in every capacity, >= the sum of its big pieces, 0 for bad capacities
+    w0 = lib.ovl_workspace_bytes(dims, B.OVL_F64, B.OVL_RECON18, 0, 1, 0)
+    assert w0 == lib.ovl_device_bytes(dims, B.OVL_F64, B.OVL_RECON18, 0)
+    assert w0 >= v * (4 * 9 * 16 + 10 * 12 * 16 + 2 * 12 * 16)
+    w50 = lib.ovl_workspace_bytes(dims, B.OVL_F64, B.OVL_RECON18, 50, 1, 0)
+    assert w50 - w0 >= 50 * v * 12 * 16 and w50 == got
+    w12 = lib.ovl_workspace_bytes(dims, B.OVL_F64, B.OVL_RECON18, 50, 12, 0)
+    assert w12 - w50 >= (8 * 11 + 2 * 12) * v * 12 * 16
+    we = lib.ovl_workspace_bytes(dims, B.OVL_F64, B.OVL_RECON18, 50, 12, 104)
+    assert we - w12 >= 5 * 104 * v * 12 * 16
+    assert lib.ovl_workspace_bytes(dims, B.OVL_F32, B.OVL_RECON12, 0, 1, 0) < w0 // 2 + 2 * v * 12 * 16
+    for bad_caps in [(-1, 1, 0), (0, 0, 0), (0, 13, 0), (0, 1, -1), (0, 1, 129)]:
+        assert lib.ovl_workspace_bytes(dims, B.OVL_F64, B.OVL_RECON18, *bad_caps) == 0
     ctx = ctypes.c_void_p()
+    assert lib.ovl_create_ws(ctypes.byref(ctx), dims, ctypes.c_void_p(16), B.OVL_F64, B.OVL_RECON18, 0, 1, 0, None, 0, None) == B.OVL_EINVAL
     assert lib.ovl_create(ctypes.byref(ctx), bad, ctypes.c_void_p(16), B.OVL_F64, B.OVL_RECON18, None) == B.OVL_EINVAL
     assert lib.ovl_create(ctypes.byref(ctx), dims, None, B.OVL_F64, B.OVL_RECON18, None) == B.OVL_EINVAL
     assert lib.ovl_destroy(None) == B.OVL_EINVAL

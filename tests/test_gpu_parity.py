@@ -665,3 +665,71 @@ def test_eigensolver_not_converged_returns_consistent_ritz_pairs(torch, api, orc
                 r = np.linalg.norm((kp - lam[i] * ph[i]).ravel())
                 assert abs(r - res[i]) <= 1e-9 + 1e-6 * res[i], (cycles, i, r, res[i], ok)
                 assert abs(np.linalg.norm(ph[i].ravel()) - 1.0) < 1e-10
+
+
+def test_caller_owned_workspace(torch, api, orc):
+    """a context created inside a torch-owned workspace (ovl_create_ws) never allocates or frees device memory
+    afterwards -- torch's allocator sees every byte -- and gives results bit-identical to the library-owned context.
+    Exceeding a capacity the workspace was sized for is OVL_EINVAL, not a hidden allocation."""
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 6, 8)
+    U = inputs.config_links(dims, 0.3, 41, stout_steps=1)
+    alpha = inputs.chebyshev_sign_coeffs(41, 0.09)
+    phi = inputs.orthonormal_vectors(dims, 4, 43)
+    lam = np.array([0.45, -0.47, 0.5, -0.52])
+    psi = np.stack([inputs.gaussian_spinor(dims, 50 + r) for r in range(3)])
+    Ud, phid, pd = dev(torch, U), dev(torch, phi), dev(torch, psi)
+    need = B.ovl_workspace_bytes(dims, B.OVL_F64, B.OVL_RECON18, 4, 3, 12)
+    assert need > 0
+    ws = torch.empty(need + 512, dtype=torch.uint8, device="cuda")
+    with api.Overlap(dims, Ud) as ref, api.Overlap(dims, Ud, workspace=dict(max_nev=4, max_rhs=3, eig_block=12, buffer=ws)) as op:
+        for o in (ref, op):
+            o.set_chebyshev(alpha)
+            o.set_deflation(phid, lam)
+        torch.cuda.synchronize()
+        free0, _ = torch.cuda.mem_get_info()
+        alloc0 = torch.cuda.memory_allocated()
+        outs = torch.empty_like(pd)
+        x = torch.empty_like(pd)
+        xs = torch.empty_like(pd[0])
+        ev = torch.empty((4, int(np.prod(dims)), 4, 3), dtype=torch.complex128, device="cuda")
+        alloc1 = torch.cuda.memory_allocated()
+        torch.cuda.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        # every entry point that used to allocate lazily: multi-rhs, CG, multi-CG, host-pointer staging, the eigensolver
+        B.ovl_overlap_multi(op.ctx, 3, 0.05, 0, pd, outs)
+        B.ovl_cg(op.ctx, 0.2, pd[0], xs, 1e-9, 200)
+        B.ovl_cg_multi(op.ctx, 3, 0.2, pd, x, 1e-9, 200)
+        hy = op.overlap(psi[1], 0.05)                      # numpy in / out: staged through the workspace
+        rc, lam_e, res_e, cyc = B.ovl_lowest_eigenpairs(op.ctx, 4, 1e-9, 30, 12, 12, ev)
+        torch.cuda.synchronize()
+        free2, _ = torch.cuda.mem_get_info()
+        assert torch.cuda.memory_allocated() == alloc1
+        assert free2 == free1, "the library allocated device memory behind torch's back"
+        assert rc == B.OVL_OK
+        # same results as the library-owned context, bit for bit
+        assert torch.equal(outs, ref.overlap_multi(pd, 0.05))
+        xr, itr, _, _ = ref.cg(pd[0], 0.2, tol=1e-9, maxiter=200)
+        assert torch.equal(xs, xr)
+        assert np.array_equal(hy, ref.overlap(psi[1], 0.05))
+        pr, lr, _, _, okr = ref.lowest_eigenpairs(4, tol=1e-9, max_cycles=30, filter_degree=12, block=12)
+        assert okr and np.array_equal(lam_e, lr) and torch.equal(ev, pr)
+        # capacities are hard limits
+        five = dev(torch, inputs.orthonormal_vectors(dims, 5, 44))
+        with pytest.raises(B.OvlError) as e:
+            op.set_deflation(five, np.array([0.4, -0.4, 0.5, -0.5, 0.6]))
+        assert e.value.code == B.OVL_EINVAL
+        four = torch.cat([pd, pd[:1]])
+        with pytest.raises(B.OvlError) as e:
+            op.overlap_multi(four, 0.05)
+        assert e.value.code == B.OVL_EINVAL
+        with pytest.raises(B.OvlError) as e:
+            op.lowest_eigenpairs(4, block=16)
+        assert e.value.code == B.OVL_EINVAL
+        assert torch.equal(op.overlap(pd[0], 0.05), ref.overlap(pd[0], 0.05))  # still usable after the errors
+    # a too small or misaligned workspace is refused
+    with pytest.raises(B.OvlError):
+        B.ovl_create_ws(dims, Ud, ws[: need - 256], max_nev=4, max_rhs=3, eig_block=12)
+    with pytest.raises(B.OvlError):
+        B.ovl_create_ws(dims, Ud, ws[8:], max_nev=4, max_rhs=3, eig_block=12)
+    assert float(np.abs(host(outs)).max()) > 0
