@@ -318,11 +318,12 @@ int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda
     for (int i = 0; i < nev; ++i)
         if (!std::isfinite(lambda[i]) || std::fabs(lambda[i]) < 1e-14 * c->lambda_max)
             return fail(c, OVL_EINVAL, "lambda[%d] = %g is zero or not finite (reading R9)", i, lambda[i]);
+    if (nev > c->proj_cap && c->ws_mode)  // refused before any state changes: the current deflation space stays in force
+        return fail(c, OVL_EINVAL, "%d eigenvectors exceed the workspace capacity max_nev = %d", nev, c->max_nev);
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     c->nev = 0;
     if (nev == 0) return OVL_OK;
     if (nev > c->proj_cap) {
-        if (c->ws_mode) return fail(c, OVL_EINVAL, "%d eigenvectors exceed the workspace capacity max_nev = %d", nev, c->max_nev);
         dev_release(c, &c->phi);
         dev_release(c, (void **)&c->proj_partial);
         dev_release(c, (void **)&c->w_dev);
