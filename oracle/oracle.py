@@ -41,6 +41,7 @@ def _load():
         _lib.orc_cheb_scalar.restype = _c.c_double
         _lib.orc_cheb_scalar.argtypes = [_c.c_int, _c.c_void_p, _c.c_double]
         _lib.orc_cg.restype = _c.c_int
+        _lib.orc_cg_chiral.restype = _c.c_int
         _lib.orc_num_threads.restype = _c.c_int
     return _lib
 
@@ -153,6 +154,31 @@ def cg(dims, U, alpha, mu, b, tol, maxiter, phi=None, lam=(), m_w=1.5, lambda_ma
     it = _load().orc_cg(_dims(dims), _p(U), _c.c_double(m_w), _c.c_double(lambda_max), _c.c_int(len(alpha) - 1),
                         _p(alpha), _c.c_int(nev), _p(phi), _p(lam), _c.c_double(mu), _p(b), _p(x),
                         _c.c_double(tol), _c.c_int(maxiter), _c.byref(rel))
+    return x, int(it), float(rel.value)
+
+
+def chiral_op(dims, U, alpha, mu, chirality, v, phi=None, lam=(), m_w=1.5, lambda_max=6.5):
+    """A_c v = 1/2 (1+mu^2) P_c v + c/2 (1-mu^2) P_c sign(K) P_c v  (reading R23)."""
+    vv = _vol(dims)
+    U = _in(U, (vv, 4, 3, 3)); v = _in(v, (vv, 4, 3)); alpha = _alpha(alpha)
+    nev, phi, lam = _defl(dims, phi, lam)
+    out = np.empty_like(v)
+    _load().orc_chiral_op(_dims(dims), _p(U), _c.c_double(m_w), _c.c_double(lambda_max), _c.c_int(len(alpha) - 1),
+                          _p(alpha), _c.c_int(nev), _p(phi), _p(lam), _c.c_double(mu), _c.c_int(int(chirality)),
+                          _p(v), _p(out))
+    return out
+
+
+def cg_chiral(dims, U, alpha, mu, chirality, b, tol, maxiter, phi=None, lam=(), m_w=1.5, lambda_max=6.5):
+    """CG on A_c x = P_c b in the chirality sector. Returns (x, iterations, true relative residual)."""
+    v = _vol(dims)
+    U = _in(U, (v, 4, 3, 3)); b = _in(b, (v, 4, 3)); alpha = _alpha(alpha)
+    nev, phi, lam = _defl(dims, phi, lam)
+    x = np.empty_like(b)
+    rel = _c.c_double(0.0)
+    it = _load().orc_cg_chiral(_dims(dims), _p(U), _c.c_double(m_w), _c.c_double(lambda_max), _c.c_int(len(alpha) - 1),
+                               _p(alpha), _c.c_int(nev), _p(phi), _p(lam), _c.c_double(mu), _c.c_int(int(chirality)),
+                               _p(b), _p(x), _c.c_double(tol), _c.c_int(maxiter), _c.byref(rel))
     return x, int(it), float(rel.value)
 
 

@@ -16,6 +16,9 @@
  *   orc_sign      eq. 2.3 complete
  *   orc_overlap   eq. 2.1 and its adjoint                               (R12)
  *   orc_cg        textbook Hestenes-Stiefel CG on D^dag D (north_star (d); R13, R14)
+ *   orc_chiral_op, orc_cg_chiral
+ *                 the chiral-sector form of D^dag D ("[D^dag D, gamma5] = 0": one sign
+ *                 application per operator application) and the same textbook CG on it          (R23)
  *
  * Conventions: dims = {Lx,Ly,Lz,Lt}; site s = x + Lx (y + Ly (z + Lz t));
  * links U[s][mu][row][col], mu = x,y,z,t, U_mu(x) is the matrix multiplying psi(x + mu) in eq. 2.2;
@@ -24,7 +27,8 @@
  * gamma5 = gamma_x gamma_y gamma_z gamma_t = diag(1,1,-1,-1).
  *
  * Parity pins: tests/test_oracle_*.py (closed-form free spectrum, gamma5-hermiticity, gauge covariance,
- * dense eigendecomposition on 2^4/4^4, sign^2 = 1, Ginsparg-Wilson, dense CG solve).  Nothing here is
+ * dense eigendecomposition on 2^4/4^4, sign^2 = 1, Ginsparg-Wilson, dense CG solve; the chiral-sector
+ * operator against P_c D^dag D P_c built from the dense exact sign function).  Nothing here is
  * "parity unpinned" except what is tied to the paper's ensembles and timings (unavailable).
  *
  * Loops over sites are OpenMP-parallel; there is no blocking, fusion or reordering beyond that.
@@ -252,5 +256,74 @@ int orc_cg(const int *dims, const cplx *U, double m_w, double lambda_max, int N,
     for (long i = 0; i < n; ++i) Ap[i] = b[i] - Ap[i];
     *true_relres = sqrt(norm2(n, Ap) / bb);
     free(r); free(p); free(q); free(Ap);
+    return it;
+}
+
+/* Chiral-sector operator (reading R23).  With P_c = (1 + c gamma5)/2, c = +1 or -1, and s = sign(K):
+ *   D^dag D = 1/4 [ (1+mu)^2 + (1-mu)^2 s^2 + (1-mu^2) (gamma5 s + s gamma5) ]           from eq. 2.1 and its adjoint,
+ *   s^2 = 1  =>  D^dag D = 1/2 (1+mu^2) + 1/4 (1-mu^2) {gamma5, s},  which commutes with gamma5, and
+ *   P_c D^dag D P_c = [ 1/2 (1+mu^2) + c/2 (1-mu^2) P_c s P_c ] P_c .
+ * This routine applies  A_c v = 1/2 (1+mu^2) P_c v + c/2 (1-mu^2) P_c s P_c v   with ONE evaluation of eq. 2.3
+ * (the full D^dag D needs two).  For the polynomial s of eq. 2.3, A_c differs from P_c D^dag D P_c by
+ * 1/4 (1-mu)^2 P_c (s^2 - 1) P_c.  `v` need not be chiral: it is projected first. */
+void orc_chiral_op(const int *dims, const cplx *U, double m_w, double lambda_max, int N, const double *alpha, int nev,
+                   const cplx *phi, const double *lambda, double mu, int chirality, const cplx *v, cplx *out) {
+    const long V = vol(dims), n = V * 12;
+    const double c = chirality >= 0 ? 1.0 : -1.0;
+    cplx *pv = malloc(sizeof(cplx) * n), *sg = malloc(sizeof(cplx) * n);
+    for (long s = 0; s < V; ++s)
+        for (int a = 0; a < 4; ++a)
+            for (int k = 0; k < 3; ++k) {
+                long i = (s * 4 + a) * 3 + k;
+                pv[i] = 0.5 * (1.0 + c * GAMMA5[a]) * v[i];          /* P_c v */
+            }
+    orc_sign(dims, U, m_w, lambda_max, N, alpha, nev, phi, lambda, pv, sg);
+    for (long s = 0; s < V; ++s)
+        for (int a = 0; a < 4; ++a)
+            for (int k = 0; k < 3; ++k) {
+                long i = (s * 4 + a) * 3 + k;
+                cplx ps = 0.5 * (1.0 + c * GAMMA5[a]) * sg[i];       /* P_c s P_c v */
+                out[i] = 0.5 * (1.0 + mu * mu) * pv[i] + 0.5 * c * (1.0 - mu * mu) * ps;
+            }
+    free(pv); free(sg);
+}
+
+/* CG on A_c x = P_c b in the chirality-c subspace, x0 = 0; same stopping rule as orc_cg.  Returns iterations;
+ * *true_relres = || P_c b - A_c x || / || P_c b ||.  (P_c b = 0: x = 0, zero iterations.) */
+int orc_cg_chiral(const int *dims, const cplx *U, double m_w, double lambda_max, int N, const double *alpha, int nev,
+                  const cplx *phi, const double *lambda, double mu, int chirality, const cplx *b, cplx *x, double tol,
+                  int maxiter, double *true_relres) {
+    const long V = vol(dims), n = V * 12;
+    const double c = chirality >= 0 ? 1.0 : -1.0;
+    cplx *bc = malloc(sizeof(cplx) * n), *r = malloc(sizeof(cplx) * n), *p = malloc(sizeof(cplx) * n),
+         *Ap = malloc(sizeof(cplx) * n);
+    for (long s = 0; s < V; ++s)
+        for (int a = 0; a < 4; ++a)
+            for (int k = 0; k < 3; ++k) {
+                long i = (s * 4 + a) * 3 + k;
+                bc[i] = 0.5 * (1.0 + c * GAMMA5[a]) * b[i];
+            }
+    memset(x, 0, sizeof(cplx) * n);
+    memcpy(r, bc, sizeof(cplx) * n);
+    memcpy(p, bc, sizeof(cplx) * n);
+    const double bb = norm2(n, bc);
+    double rr = bb;
+    int it = 0;
+    while (bb > 0 && it < maxiter && !(tol > 0 && sqrt(rr) <= tol * sqrt(bb))) {
+        orc_chiral_op(dims, U, m_w, lambda_max, N, alpha, nev, phi, lambda, mu, chirality, p, Ap);
+        cplx pAp = 0;
+        for (long i = 0; i < n; ++i) pAp += conj(p[i]) * Ap[i];
+        const double a = rr / creal(pAp);
+        for (long i = 0; i < n; ++i) { x[i] += a * p[i]; r[i] -= a * Ap[i]; }
+        const double rr_new = norm2(n, r);
+        const double beta = rr_new / rr;
+        for (long i = 0; i < n; ++i) p[i] = r[i] + beta * p[i];
+        rr = rr_new;
+        ++it;
+    }
+    orc_chiral_op(dims, U, m_w, lambda_max, N, alpha, nev, phi, lambda, mu, chirality, x, Ap);
+    for (long i = 0; i < n; ++i) Ap[i] = bc[i] - Ap[i];
+    *true_relres = bb > 0 ? sqrt(norm2(n, Ap) / bb) : 0.0;
+    free(bc); free(r); free(p); free(Ap);
     return it;
 }

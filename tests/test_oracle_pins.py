@@ -321,6 +321,92 @@ def test_cg_against_dense_solve(orc, dense44):
     assert all(e1 > e2 for e1, e2 in zip(errs, errs[1:]))
 
 
+# ---------------------------------------------------------------- chiral-sector D^dag D (reading R23)
+
+def test_chiral_sector_operator_dense(orc, dense44):
+    """orc_chiral_op against the plain definition: P_c D^dag D P_c with D = 1/2 (1 + mu + (1 - mu) gamma5 S) built densely
+    from the EXACT sign matrix S of the eigendecomposition (S^2 = 1).  With a delta ~ 1e-13 polynomial the two agree to
+    1e-11: pins the constants 1/2 (1 + mu^2), c/2 (1 - mu^2), both chiralities and the projections; D^dag D commutes
+    with gamma5."""
+    d = dense44
+    dims, U = d["dims"], d["U"]
+    n = d["K"].shape[0]
+    alpha = inputs.chebyshev_sign_coeffs(401, 0.95 * np.abs(d["lam"]).min() / 6.5)
+    G5m = np.tile(np.repeat(G5, 3), n // 12)
+    v = inputs.gaussian_spinor(dims, 67)  # NOT chiral: the routine projects
+    for mu in (0.0, 0.05, 0.3):
+        Dex = 0.5 * ((1 + mu) * np.eye(n) + (1 - mu) * (G5m[:, None] * d["S"]))
+        A = Dex.conj().T @ Dex
+        assert np.abs(A * G5m[None, :] - G5m[:, None] * A).max() < 1e-12      # [D^dag D, gamma5] = 0 for the exact sign
+        for c in (+1, -1):
+            Pc = 0.5 * (1 + c * G5m)
+            want = Pc * (A @ (Pc * v.ravel()))
+            got = orc.chiral_op(dims, U, alpha, mu, c, v)
+            assert rel_err(got.ravel(), want) < 1e-11
+            assert np.abs((1 - Pc) * got.ravel()).max() == 0.0                 # stays in the sector exactly
+            # and against the oracle's own two-apply D^dag D on a chiral vector
+            pv = (Pc * v.ravel()).reshape(v.shape)
+            two = orc.overlap(dims, U, alpha, mu, orc.overlap(dims, U, alpha, mu, pv), dagger=True)
+            assert rel_err(got, two) < 1e-11
+
+
+def test_chiral_sector_error_term(orc, dense44):
+    """With a POOR polynomial (delta = max |p(lambda^) - sign| over the dense spectrum) the sector operator differs from
+    P_c D^dag D P_c (the oracle's two applies, same polynomial) by exactly 1/4 (1 - mu)^2 P_c (s^2 - 1) P_c: norm <=
+    1/4 (1 - mu)^2 (2 delta + delta^2) ||v||, and it is not accidentally zero."""
+    d = dense44
+    dims, U = d["dims"], d["U"]
+    n = d["K"].shape[0]
+    alpha = inputs.chebyshev_sign_coeffs(41, 0.95 * np.abs(d["lam"]).min() / 6.5)
+    delta = np.abs(inputs.chebyshev_eval(alpha, d["lam"] / 6.5) - np.sign(d["lam"])).max()
+    assert 1e-4 < delta < 0.5
+    G5m = np.tile(np.repeat(G5, 3), n // 12)
+    mu = 0.1
+    for c in (+1, -1):
+        Pc = 0.5 * (1 + c * G5m)
+        pv = (Pc * inputs.gaussian_spinor(dims, 68).ravel()).reshape(-1, 4, 3)
+        two = orc.overlap(dims, U, alpha, mu, orc.overlap(dims, U, alpha, mu, pv), dagger=True)
+        got = orc.chiral_op(dims, U, alpha, mu, c, pv)
+        diff = np.linalg.norm(Pc * two.ravel() - got.ravel()) / np.linalg.norm(pv.ravel())
+        assert 1e-8 < diff <= 0.25 * (1 - mu) ** 2 * (2 * delta + delta * delta) * 1.0000001
+        # the predicted form of the difference, through the oracle's own sign function
+        s2 = orc.sign(dims, U, alpha, orc.sign(dims, U, alpha, pv))
+        pred = 0.25 * (1 - mu) ** 2 * (Pc * (s2.ravel() - pv.ravel()))
+        assert rel_err(Pc * two.ravel() - got.ravel(), pred) < 1e-9
+
+
+def test_cg_chiral_against_dense_solve(orc, dense44):
+    """orc_cg_chiral vs numpy's dense solve of the sector system built from the SAME polynomial (so the comparison is
+    limited by the CG tolerance only), and vs the full D^dag D solve on a chiral source (limited by kappa * delta)."""
+    d = dense44
+    dims, U = d["dims"], d["U"]
+    n = d["K"].shape[0]
+    mu = 0.05
+    alpha = inputs.chebyshev_sign_coeffs(101, 0.95 * np.abs(d["lam"]).min() / 6.5)
+    pl = inputs.chebyshev_eval(alpha, d["lam"] / 6.5)
+    Sp = (d["W"] * pl) @ d["W"].conj().T
+    G5m = np.tile(np.repeat(G5, 3), n // 12)
+    b = inputs.gaussian_spinor(dims, 92)
+    for c in (+1, -1):
+        Pc = 0.5 * (1 + c * G5m)
+        idx = np.nonzero(Pc)[0]
+        Ac = 0.5 * (1 + mu * mu) * np.eye(len(idx)) + 0.5 * c * (1 - mu * mu) * Sp[np.ix_(idx, idx)]
+        xs = np.zeros(n, complex)
+        xs[idx] = np.linalg.solve(Ac, b.ravel()[idx])
+        x, it, rel = orc.cg_chiral(dims, U, alpha, mu, c, b, 1e-10, 500)
+        assert 5 < it < 500 and rel < 1.5e-10
+        assert np.abs((1 - Pc) * x.ravel()).max() == 0.0
+        assert np.linalg.norm(x.ravel() - xs) / np.linalg.norm(xs) < 1e-7
+        # the full operator on the chiral source: same solution up to the polynomial's s^2 - 1 (delta ~ 3e-5 here)
+        xf, _, _ = orc.cg(dims, U, alpha, mu, (Pc * b.ravel()).reshape(b.shape), 1e-10, 500)
+        assert np.linalg.norm(xf.ravel() - x.ravel()) / np.linalg.norm(x.ravel()) < 1e-2
+        # fixed iteration count honoured; zero sector source -> zero iterations
+        xk, itk, _ = orc.cg_chiral(dims, U, alpha, mu, c, b, 0.0, 7)
+        assert itk == 7
+        x0, it0, rel0 = orc.cg_chiral(dims, U, alpha, mu, c, ((1 - Pc) * b.ravel()).reshape(b.shape), 1e-10, 50)
+        assert it0 == 0 and rel0 == 0.0 and not x0.any()
+
+
 # ---------------------------------------------------------------- input generators
 
 def test_links_unitary_and_smearing_raises_plaquette():
