@@ -152,6 +152,15 @@ int ovl_overlap_multi(ovl_ctx *ctx, int nrhs, double mu, int dagger, const void 
 int ovl_cg(ovl_ctx *ctx, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out,
            double *true_relres_out);
 
+/* CG in one chirality sector ("[D^dag D, gamma5] = 0", one sign application per operator
+ * application instead of two; reading R23).  With P_c = (1 + c gamma5)/2, c = chirality = +1 or -1, solves
+ *     A_c x = P_c b,   A_c = 1/2 (1 + mu^2) + c/2 (1 - mu^2) P_c sign(K) P_c     ( = P_c D^dag D P_c when sign(K)^2 = 1;
+ * for the polynomial of eq. 2.3 the two differ by 1/4 (1-mu)^2 P_c (sign(K)^2 - 1) P_c ),  x0 = 0, same stopping rule and
+ * outputs as ovl_cg; x = P_c x.  *true_relres_out = ||P_c b - A_c x|| / ||P_c b||.  b need not be chiral (it is projected);
+ * P_c b = 0 returns x = 0 after 0 iterations.  Errors as ovl_cg; OVL_EINVAL for chirality not +-1.  Synchronises. */
+int ovl_cg_chiral(ovl_ctx *ctx, double mu, int chirality, const void *b, void *x, double tol, int maxiter, int *iters_out,
+                  double *true_relres_out);
+
 /* nrhs independent systems D^dag D x_r = b_r solved in lockstep (1 <= nrhs <= OVL_MAX_RHS): every operator application
  * is one multi-right-hand-side call (see ovl_overlap_multi), alpha, beta and the residual norms are kept per system; a
  * system that has reached tol is frozen while the others iterate.  b, x [H|D]: [nrhs][V][4][3]; iters_out, true_relres_out:

@@ -117,6 +117,13 @@ class Overlap:
         rc, it, rel = B.ovl_cg(self.ctx, mu, b, x, tol, maxiter)
         return x, it, rel, rc == B.OVL_OK
 
+    def cg_chiral(self, b, mu, chirality, tol=1e-8, maxiter=1000):
+        """Solve A_c x = P_c b in the chirality sector (one sign application per iteration instead of two; reading R23).
+        Returns (x, iterations, true relative residual, converged)."""
+        x = self._like(b)
+        rc, it, rel = B.ovl_cg_chiral(self.ctx, mu, chirality, b, x, tol, maxiter)
+        return x, it, rel, rc == B.OVL_OK
+
     def cg_multi(self, b, mu, tol=1e-8, maxiter=1000):
         """b: (nrhs, V, 4, 3). Solve D^dag D x_r = b_r in lockstep. Returns (x, iterations[], true relres[], converged)."""
         x = self._like(b)

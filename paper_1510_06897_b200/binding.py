@@ -42,6 +42,7 @@ SIGNATURES = {
     "ovl_overlap": (_I, [_P, _D, _I, _P, _P]),
     "ovl_overlap_multi": (_I, [_P, _I, _D, _I, _P, _P]),
     "ovl_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_cg_chiral": (_I, [_P, _D, _I, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_multi": (_I, [_P, _I, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_mixed": (_I, [_P, _P, _D, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
     "ovl_lowest_eigenpairs": (_I, [_P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I)]),
@@ -205,6 +206,15 @@ def ovl_cg(ctx, mu, b, x, tol, maxiter):
     """Returns (status, iterations, true relative residual); status is OVL_OK or OVL_ENOTCONV."""
     it, rel = _I(0), _D(0.0)
     rc = load_library().ovl_cg(ctx, float(mu), _ptr(b), _ptr(x), float(tol), int(maxiter), C.byref(it), C.byref(rel))
+    _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, int(it.value), float(rel.value)
+
+
+def ovl_cg_chiral(ctx, mu, chirality, b, x, tol, maxiter):
+    """Returns (status, iterations, true relative residual) of the chiral-sector solve A_c x = P_c b."""
+    it, rel = _I(0), _D(0.0)
+    rc = load_library().ovl_cg_chiral(ctx, float(mu), int(chirality), _ptr(b), _ptr(x), float(tol), int(maxiter),
+                                      C.byref(it), C.byref(rel))
     _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
     return rc, int(it.value), float(rel.value)
 

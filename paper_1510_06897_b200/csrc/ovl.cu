@@ -380,6 +380,21 @@ int ovl_cg(ovl_ctx *c, double mu, const void *b, void *x, double tol, int maxite
     return rc;
 }
 
+int ovl_cg_chiral(ovl_ctx *c, double mu, int chirality, const void *b, void *x, double tol, int maxiter, int *iters_out,
+                  double *relres_out) {
+    if (!c) return OVL_EINVAL;
+    if (!b || !x || b == x || !iters_out || !relres_out || maxiter < 0 || (chirality != 1 && chirality != -1))
+        return fail(c, OVL_EINVAL, "bad ovl_cg_chiral arguments (chirality must be +1 or -1)");
+    if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
+    OVL_TRY(import_any(c, b, c->psi_n));
+    int rc = DISPATCH(c, cg_native, c, mu, c->psi_n, c->out_n, tol, maxiter, iters_out, relres_out, 1, chirality);
+    if (rc != OVL_OK && rc != OVL_ENOTCONV) return rc;
+    int rc2 = export_any(c, c->out_n, x);
+    if (rc2 != OVL_OK) return rc2;
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    return rc;
+}
+
 int ovl_cg_multi(ovl_ctx *c, int nrhs, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out, double *relres_out) {
     if (!c) return OVL_EINVAL;
     if (!b || !x || b == x || !iters_out || !relres_out || maxiter < 0) return fail(c, OVL_EINVAL, "bad ovl_cg_multi arguments");

@@ -141,9 +141,11 @@ k_project_final(int nblk, int nev, int wstride, const double2 *__restrict__ part
 template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS)
 k_deflate_assemble(size_t n, size_t n_upper, int nev, int nrhs, int wstride, const cx<T> *__restrict__ phi, const double2 *__restrict__ w,
-                   const cx<T> *__restrict__ psi, const cx<T> *__restrict__ acc, T a, T b, int g5, cx<T> *__restrict__ out) {
+                   const cx<T> *__restrict__ psi, const cx<T> *__restrict__ acc, T a, T b, int g5, int chir, cx<T> *__restrict__ out) {
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n) return;
+    // chir = +1 / -1: the result is projected with P_c = (1 + c gamma5)/2, i.e. the planes of the other chirality are zero
+    const bool dead = (chir > 0 && e >= n_upper) || (chir < 0 && e < n_upper);
     const int r0 = blockIdx.y * DEFL_RB;
     const int nr = min(DEFL_RB, nrhs - r0);
     double re[DEFL_RB], im[DEFL_RB];
@@ -175,9 +177,20 @@ k_deflate_assemble(size_t n, size_t n_upper, int nev, int nrhs, int wstride, con
             } else {
                 q.x = b * sx; q.y = b * sy;
             }
+            if (dead) q = mk<T>(0, 0);
             out[o] = q;
         }
     }
+}
+
+// out = P_c in, P_c = (1 + c gamma5)/2: zero the planes of the other chirality (blockIdx.y = right-hand side)
+template <typename T>
+__global__ void k_chiral_project(size_t n, size_t n_upper, int chir, const cx<T> *__restrict__ in, cx<T> *__restrict__ out) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    in += blockIdx.y * n; out += blockIdx.y * n;
+    const bool dead = (chir > 0 && e >= n_upper) || (chir < 0 && e < n_upper);
+    out[e] = dead ? mk<T>(0, 0) : in[e];
 }
 
 // out = gamma5 in (only used to form the input of sign() in D^dag)

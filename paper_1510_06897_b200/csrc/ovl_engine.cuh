@@ -235,7 +235,7 @@ inline int ensure_proj(ovl_ctx *c, int nrhs) {
 // (dagger = 1, gamma5 not applied on the way out).  ovl_sign uses a = 0, b = 1, g5out = 0.  The polynomial loop handles
 // all right-hand sides in every launch (links amortised); the two deflation passes read every phi_i once per group of
 // DEFL_RB right-hand sides.
-template <typename T> int sign_combine_native(ovl_ctx *c, int nrhs, double a, double b, int dagger, int g5out, const void *in, void *out) {
+template <typename T> int sign_combine_native(ovl_ctx *c, int nrhs, double a, double b, int dagger, int g5out, const void *in, void *out, int chir = 0) {
     if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
     OVL_TRY(ensure_work(c, nrhs));
     const size_t n = c->n(), n_upper = (size_t)6 * c->g.V;
@@ -259,7 +259,7 @@ template <typename T> int sign_combine_native(ovl_ctx *c, int nrhs, double a, do
     // ... and once more per group in the update + assembly pass
     k_deflate_assemble<T><<<dim3(grid_for(n, BLAS_THREADS, 1 << 30), ngrp), BLAS_THREADS, 0, c->st>>>(
         n, n_upper, c->nev, nrhs, c->proj_cap > 0 ? c->proj_cap : 1, (const cx<T> *)c->phi, c->w_dev, (const cx<T> *)in, (const cx<T> *)c->acc, (T)a,
-        (T)b, g5out, (cx<T> *)out);
+        (T)b, g5out, chir, (cx<T> *)out);
     OVL_LAUNCH_CHECK(c);
     return OVL_OK;
 }
@@ -296,14 +296,29 @@ inline int ensure_cg(ovl_ctx *c, int nrhs) {
     return OVL_OK;
 }
 
+// chir = 0: A = D^dag D (two sign applications per operator application).  chir = +1 / -1: the chiral-sector system
+// A_c x = P_c b,  A_c = 1/2 (1+mu^2) + c/2 (1-mu^2) P_c sign(K) P_c  (reading R23; = P_c D^dag D P_c for sign(K)^2 = 1):
+// ONE sign application per operator application; every CG vector stays in the chirality sector.
 template <typename T>
-int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int maxiter, int *iters, double *relres, int nrhs = 1) {
-    const size_t n = c->n(), fb = c->field_bytes() * nrhs;
+int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int maxiter, int *iters, double *relres, int nrhs = 1,
+              int chir = 0) {
+    const size_t n = c->n(), fb = c->field_bytes() * nrhs, n_upper = (size_t)6 * c->g.V;
     OVL_TRY(ensure_cg(c, nrhs));
+    const dim3 gride(grid_for(n, BLAS_THREADS, 1 << 30), nrhs);
+    auto apply_A = [&](const void *in, void *out) -> int {
+        if (chir) return sign_combine_native<T>(c, nrhs, 0.5 * (1.0 + mu * mu), 0.5 * chir * (1.0 - mu * mu), 0, 0, in, out, chir);
+        OVL_TRY(overlap_native<T>(c, mu, 0, in, c->cg_q, nrhs));
+        return overlap_native<T>(c, mu, 1, c->cg_q, out, nrhs);
+    };
     OVL_CUDA(c, cudaMemsetAsync(x_n, 0, fb, c->st));
-    OVL_CUDA(c, cudaMemcpyAsync(c->cg_r, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
-    OVL_CUDA(c, cudaMemcpyAsync(c->cg_p, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
-    OVL_TRY(reduce_redot<T>(c, b_n, b_n, 0, nrhs));
+    if (chir) {
+        k_chiral_project<T><<<gride, BLAS_THREADS, 0, c->st>>>(n, n_upper, chir, (const cx<T> *)b_n, (cx<T> *)c->cg_r);
+        OVL_LAUNCH_CHECK(c);
+    } else {
+        OVL_CUDA(c, cudaMemcpyAsync(c->cg_r, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
+    }
+    OVL_CUDA(c, cudaMemcpyAsync(c->cg_p, c->cg_r, fb, cudaMemcpyDeviceToDevice, c->st));
+    OVL_TRY(reduce_redot<T>(c, c->cg_r, c->cg_r, 0, nrhs));
     OVL_TRY(fetch_scalars(c, nrhs));
     double bb[OVL_MAX_RHS], rr[OVL_MAX_RHS];
     bool conv[OVL_MAX_RHS];
@@ -334,8 +349,7 @@ int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int
         return OVL_OK;
     };
     while (enq < maxiter && nconv < nrhs) {
-        OVL_TRY(overlap_native<T>(c, mu, 0, c->cg_p, c->cg_q, nrhs));
-        OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap, nrhs));
+        OVL_TRY(apply_A(c->cg_p, c->cg_Ap));
         OVL_TRY(reduce_redot<T>(c, c->cg_p, c->cg_Ap, 1, nrhs));  // alpha = rr / Re(p^dag A p)
         k_cg_update<T><<<gridr, BLAS_THREADS, 0, c->st>>>(n, c->sc_dev, (const cx<T> *)c->cg_p, (const cx<T> *)c->cg_Ap,
                                                         (cx<T> *)x_n, (cx<T> *)c->cg_r, c->red_partial);
@@ -352,11 +366,14 @@ int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int
     }
     while (seen < enq && nconv < nrhs) OVL_TRY(check(seen++));
     const int it = enq;
-    // true residuals ||b - A x|| / ||b||
-    OVL_TRY(overlap_native<T>(c, mu, 0, x_n, c->cg_q, nrhs));
-    OVL_TRY(overlap_native<T>(c, mu, 1, c->cg_q, c->cg_Ap, nrhs));
+    // true residuals ||b - A x|| / ||b||   (chiral: || P_c (b - A_c x) || / || P_c b ||)
+    OVL_TRY(apply_A(x_n, c->cg_Ap));
     k_sub<T><<<gridv, BLAS_THREADS, 0, c->st>>>(n, (const cx<T> *)b_n, (const cx<T> *)c->cg_Ap, (cx<T> *)c->cg_q);
     OVL_LAUNCH_CHECK(c);
+    if (chir) {
+        k_chiral_project<T><<<gride, BLAS_THREADS, 0, c->st>>>(n, n_upper, chir, (const cx<T> *)c->cg_q, (cx<T> *)c->cg_q);
+        OVL_LAUNCH_CHECK(c);
+    }
     OVL_TRY(reduce_redot<T>(c, c->cg_q, c->cg_q, 3, nrhs));
     OVL_TRY(fetch_scalars(c, nrhs));
     for (int r = 0; r < nrhs; ++r) relres[r] = bb[r] > 0 ? std::sqrt(c->sc_host[r * SC_N + SC_PAP] / bb[r]) : 0.0;

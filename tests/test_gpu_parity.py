@@ -733,3 +733,60 @@ def test_caller_owned_workspace(torch, api, orc):
     with pytest.raises(B.OvlError):
         B.ovl_create_ws(dims, Ud, ws[8:], max_nev=4, max_rhs=3, eig_block=12)
     assert float(np.abs(host(outs)).max()) > 0
+
+
+@pytest.mark.parametrize("chir", [+1, -1])
+def test_cg_chiral_sector(torch, api, orc, chir):
+    """ovl_cg_chiral (reading R23) against the oracle's chiral-sector CG: fixed iterations at 1e-10, to
+    tolerance (R14's checks), solution confined to the sector, half the stencil launches of the full D^dag D solve, and
+    agreement with the full solve on the projected source up to the polynomial's s^2 - 1."""
+    dims = (4, 4, 6, 8)
+    U = inputs.config_links(dims, 0.3, 21, stout_steps=2)
+    alpha = inputs.chebyshev_sign_coeffs(161, 0.07)     # delta ~ 1e-6 on this spectrum
+    phi = inputs.orthonormal_vectors(dims, 3, 23)
+    lam = np.array([0.5, -0.51, 0.52])
+    b = inputs.gaussian_spinor(dims, 24)
+    mu = 0.1
+    g5v = G5[None, :, None]
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        bd = dev(torch, b)
+        xk, itk, _, okk = op.cg_chiral(bd, mu, chir, tol=0.0, maxiter=8)
+        l0 = op.launch_count()
+        x, it, rel, ok = op.cg_chiral(bd, mu, chir, tol=1e-9, maxiter=500)
+        l1 = op.launch_count()
+        pb = dev(torch, 0.5 * (1 + chir * g5v) * b)
+        xf, itf, relf, okf = op.cg(pb, mu, tol=1e-9, maxiter=500)
+        l2 = op.launch_count()
+    wk, ito, _ = orc.cg_chiral(dims, U, alpha, mu, chir, b, 0.0, 8, phi, lam)
+    assert itk == ito == 8 and okk
+    assert rel_err(host(xk), wk) < TOL_OVL
+    xo, ito, relo = orc.cg_chiral(dims, U, alpha, mu, chir, b, 1e-9, 500, phi, lam)
+    assert ok and abs(it - ito) <= 2 and rel < 1.05e-9 and relo < 1.05e-9
+    assert rel_err(host(x), xo) < 1e-6
+    assert np.abs(0.5 * (1 - chir * g5v) * host(x)).max() == 0.0            # x = P_c x exactly
+    # one sign application per iteration instead of two
+    assert okf and abs(itf - it) <= 2
+    per_it_chiral, per_it_full = (l1 - l0) / (it + 1), (l2 - l1) / (itf + 1)
+    assert per_it_chiral < 0.55 * per_it_full
+    assert rel_err(host(xf), host(x)) < 1e-3                                # kappa * 1/4 (1-mu)^2 * 2 delta
+
+
+def test_cg_chiral_argument_checks(torch, api):
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 4, 4)
+    U = inputs.random_links(dims, 0.3, 5)
+    b = dev(torch, inputs.gaussian_spinor(dims, 6))
+    with api.Overlap(dims, dev(torch, U)) as op:
+        with pytest.raises(B.OvlError) as e:
+            op.cg_chiral(b, 0.1, +1)
+        assert e.value.code == B.OVL_ESTATE
+        op.set_chebyshev(inputs.chebyshev_sign_coeffs(21, 0.1))
+        with pytest.raises(B.OvlError) as e:
+            op.cg_chiral(b, 0.1, 0)
+        assert e.value.code == B.OVL_EINVAL
+        z = torch.zeros_like(b)
+        z[:, 2:] = b[:, 2:]                                                  # purely negative chirality
+        x0, it0, rel0, ok0 = op.cg_chiral(z, 0.1, +1, tol=1e-9, maxiter=10)
+        assert ok0 and it0 == 0 and rel0 == 0.0 and torch.count_nonzero(x0).item() == 0
