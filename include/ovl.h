@@ -196,6 +196,39 @@ int ovl_lowest_eigenpairs(ovl_ctx *ctx, int nev, double tol, int max_cycles, int
 
 const char *ovl_last_error(const ovl_ctx *ctx);
 
+/* ---- the lattice split along t over several GPUs --------------------------------------
+ * The paper ran this decomposition on 2 GPUs over MPI (PAPER.md:82-88 Table 3, :99-102 Table 4, :108).  An ovl_group is
+ * nslabs slab contexts in THIS process: slab r owns the time slices [r Lt/nslabs, (r+1) Lt/nslabs) of every field, runs
+ * on cuda_streams[r] and on device devices[r] (NULL: all on the current device -- several slabs on one GPU is the
+ * single-GPU test configuration).  There is no separate exchange step: each fused stencil launch stores the boundary
+ * time slices of its output straight into the neighbour slabs' halo buffers (peer stores over NVLink when the slabs are
+ * on different GPUs; peer access is enabled here), reads the t-neighbours of its own boundary sites from its halos, and is
+ * ordered against its two neighbours by events only (no kernel spins on a flag).  The antiperiodic t phase (reading R3)
+ * is applied by the slabs that own t = 0 and t = Lt-1.  Deflation coefficients and CG scalars are summed over slabs in slab
+ * order by every slab (peer reads).
+ * Results: D_W, K^ and the polynomial part of eq. 2.3 are BIT-IDENTICAL to the undivided lattice (same arithmetic per
+ * site); with deflation or in CG the reductions are partitioned differently and agree to rounding (~1e-15 relative).
+ * Arguments are GLOBAL canonical arrays [H|D] exactly as for the ovl_* calls of the undivided lattice (device pointers
+ * must be readable from every slab's device); slab r works on its contiguous t-range of them.  Every group call that
+ * produces a field synchronises all slab streams before returning.  Only the Clenshaw evaluation order is offered.
+ * Requirements: 1 <= nslabs <= 16, Lt % nslabs == 0, Lt / nslabs >= 2.  Errors as the corresponding ovl_* calls;
+ * ovl_group_last_error names the slab. */
+typedef struct ovl_group ovl_group;
+int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void *links_c128, int prec, int recon,
+                     void *const *cuda_streams, const int *devices);
+int ovl_group_destroy(ovl_group *g);
+int ovl_group_slabs(const ovl_group *g);
+int ovl_group_set_kernel(ovl_group *g, double m_w, double lambda_max);
+int ovl_group_set_chebyshev(ovl_group *g, int degree_N, const double *alpha);
+int ovl_group_set_deflation(ovl_group *g, int nev, const void *phi_c128, const double *lambda);
+int ovl_group_dw(ovl_group *g, const void *psi, void *out);
+int ovl_group_khat(ovl_group *g, const void *psi, void *out);
+int ovl_group_sign(ovl_group *g, const void *psi, void *out);
+int ovl_group_overlap(ovl_group *g, double mu, int dagger, const void *psi, void *out);
+int ovl_group_cg(ovl_group *g, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out, double *true_relres_out);
+const char *ovl_group_last_error(const ovl_group *g);
+long long ovl_group_launch_count(const ovl_group *g);
+
 /* ---- native-layout fields (benchmark / solver plumbing: no relayout passes inside the timed calls) -------------
  * A native field is an opaque device buffer of ovl_field_bytes(ctx) bytes owned by the caller (device memory). */
 size_t ovl_field_bytes(const ovl_ctx *ctx);

@@ -182,3 +182,80 @@ class Overlap:
 
     def launch_count(self):
         return B.ovl_launch_count(self.ctx)
+
+
+class SplitOverlap:
+    """The same operator on a lattice split along t into `nslabs` slabs (include/ovl.h, ovl_group_*): one slab per
+    stream, optionally one per GPU (devices=[...]); halo traffic is fused into the stencil kernels as peer stores.
+    Arguments and results are GLOBAL canonical fields, exactly as for Overlap."""
+
+    def __init__(self, dims, links, nslabs, prec="f64", recon=18, devices=None, m_w=1.5, lambda_max=6.5):
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1510_06897_b200 needs a CUDA device (no CPU fallback)")
+        self.dims = tuple(int(d) for d in dims)
+        self.V = int(np.prod(self.dims))
+        self.prec = B.OVL_F64 if prec in ("f64", B.OVL_F64) else B.OVL_F32
+        self.nslabs = int(nslabs)
+        self.devices = None if devices is None else [int(d) for d in devices]
+        self.streams = []
+        for r in range(self.nslabs):
+            with torch.cuda.device(self.devices[r] if self.devices else torch.cuda.current_device()):
+                self.streams.append(torch.cuda.Stream())
+        torch.cuda.synchronize()
+        self.grp = B.ovl_group_create(self.dims, self.nslabs, links, self.prec, int(recon),
+                                      [s.cuda_stream for s in self.streams], self.devices)
+        B.ovl_group_set_kernel(self.grp, m_w, lambda_max)
+        self.cdtype = torch.complex128 if self.prec == B.OVL_F64 else torch.complex64
+
+    def close(self):
+        if getattr(self, "grp", None) is not None:
+            B.ovl_group_destroy(self.grp)
+            self.grp = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def set_chebyshev(self, alpha):
+        B.ovl_group_set_chebyshev(self.grp, alpha)
+
+    def set_deflation(self, phi, lam):
+        B.ovl_group_set_deflation(self.grp, phi, lam)
+
+    def _run(self, fn, psi, *args):
+        torch = _torch()
+        torch.cuda.synchronize()  # inputs may have been produced on another stream
+        out = np.empty_like(psi) if isinstance(psi, np.ndarray) else torch.empty_like(psi)
+        fn(self.grp, *args, psi, out)
+        return out
+
+    def dw(self, psi):
+        return self._run(B.ovl_group_dw, psi)
+
+    def khat(self, psi):
+        return self._run(B.ovl_group_khat, psi)
+
+    def sign(self, psi):
+        return self._run(B.ovl_group_sign, psi)
+
+    def overlap(self, psi, mu, dagger=False):
+        return self._run(B.ovl_group_overlap, psi, mu, int(dagger))
+
+    def cg(self, b, mu, tol=1e-8, maxiter=1000):
+        torch = _torch()
+        torch.cuda.synchronize()
+        x = np.empty_like(b) if isinstance(b, np.ndarray) else torch.empty_like(b)
+        rc, it, rel = B.ovl_group_cg(self.grp, mu, b, x, tol, maxiter)
+        return x, it, rel, rc == B.OVL_OK
+
+    def launch_count(self):
+        return B.ovl_group_launch_count(self.grp)

@@ -47,6 +47,19 @@ SIGNATURES = {
     "ovl_cg_mixed": (_I, [_P, _P, _D, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
     "ovl_lowest_eigenpairs": (_I, [_P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I)]),
     "ovl_last_error": (C.c_char_p, [_P]),
+    "ovl_group_create": (_I, [C.POINTER(_P), C.POINTER(_I), _I, _P, _I, _I, C.POINTER(_P), C.POINTER(_I)]),
+    "ovl_group_destroy": (_I, [_P]),
+    "ovl_group_slabs": (_I, [_P]),
+    "ovl_group_set_kernel": (_I, [_P, _D, _D]),
+    "ovl_group_set_chebyshev": (_I, [_P, _I, C.POINTER(_D)]),
+    "ovl_group_set_deflation": (_I, [_P, _I, _P, C.POINTER(_D)]),
+    "ovl_group_dw": (_I, [_P, _P, _P]),
+    "ovl_group_khat": (_I, [_P, _P, _P]),
+    "ovl_group_sign": (_I, [_P, _P, _P]),
+    "ovl_group_overlap": (_I, [_P, _D, _I, _P, _P]),
+    "ovl_group_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_group_last_error": (C.c_char_p, [_P]),
+    "ovl_group_launch_count": (C.c_longlong, [_P]),
     "ovl_field_bytes": (C.c_size_t, [_P]),
     "ovl_field_import": (_I, [_P, _P, _P]),
     "ovl_field_export": (_I, [_P, _P, _P]),
@@ -289,3 +302,74 @@ def ovl_poly_timings(ctx, max_n=64):
 
 def ovl_launch_count(ctx) -> int:
     return int(load_library().ovl_launch_count(ctx))
+
+
+# ------------------------------------------------------------------ t-split lattice (ovl_group_*)
+
+def _gcheck(g, rc, ok=(OVL_OK,)):
+    if rc not in ok:
+        raise OvlError(rc, load_library().ovl_group_last_error(g).decode() if g else "no group")
+    return rc
+
+
+def ovl_group_create(dims, nslabs, links, prec=OVL_F64, recon=OVL_RECON18, streams=(), devices=None):
+    g = _P()
+    st = (_P * nslabs)(*[_P(int(s)) for s in streams])
+    dv = (_I * nslabs)(*map(int, devices)) if devices is not None else None
+    rc = load_library().ovl_group_create(C.byref(g), (_I * 4)(*map(int, dims)), int(nslabs), _ptr(links), prec, recon, st, dv)
+    if rc != OVL_OK:
+        raise OvlError(rc, "ovl_group_create failed")
+    return g
+
+
+def ovl_group_destroy(g):
+    return load_library().ovl_group_destroy(g)
+
+
+def ovl_group_slabs(g) -> int:
+    return int(load_library().ovl_group_slabs(g))
+
+
+def ovl_group_set_kernel(g, m_w=1.5, lambda_max=6.5):
+    return _gcheck(g, load_library().ovl_group_set_kernel(g, float(m_w), float(lambda_max)))
+
+
+def ovl_group_set_chebyshev(g, alpha):
+    a, p = _dbl(alpha)
+    return _gcheck(g, load_library().ovl_group_set_chebyshev(g, len(a) - 1, p))
+
+
+def ovl_group_set_deflation(g, phi, lam):
+    l, p = _dbl(lam)
+    return _gcheck(g, load_library().ovl_group_set_deflation(g, len(l), _ptr(phi), p))
+
+
+def ovl_group_dw(g, psi, out):
+    return _gcheck(g, load_library().ovl_group_dw(g, _ptr(psi), _ptr(out)))
+
+
+def ovl_group_khat(g, psi, out):
+    return _gcheck(g, load_library().ovl_group_khat(g, _ptr(psi), _ptr(out)))
+
+
+def ovl_group_sign(g, psi, out):
+    return _gcheck(g, load_library().ovl_group_sign(g, _ptr(psi), _ptr(out)))
+
+
+def ovl_group_overlap(g, mu, dagger, psi, out):
+    return _gcheck(g, load_library().ovl_group_overlap(g, float(mu), int(dagger), _ptr(psi), _ptr(out)))
+
+
+def ovl_group_cg(g, mu, b, x, tol, maxiter):
+    it, rel = _I(0), _D(0.0)
+    rc = load_library().ovl_group_cg(g, float(mu), _ptr(b), _ptr(x), float(tol), int(maxiter), C.byref(it), C.byref(rel))
+    _gcheck(g, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, int(it.value), float(rel.value)
+
+
+def ovl_group_last_error(g) -> str:
+    return load_library().ovl_group_last_error(g).decode()
+
+
+def ovl_group_launch_count(g) -> int:
+    return int(load_library().ovl_group_launch_count(g))

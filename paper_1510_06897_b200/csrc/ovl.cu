@@ -2,6 +2,7 @@
 // (host <-> device) and precision dispatch only; the arithmetic lives in ovl_wilson.cuh / ovl_blas.cuh.
 #include "ovl_engine.cuh"
 #include "ovl_eigsolve.cuh"
+#include "ovl_group.cuh"
 
 using namespace ovl;
 
@@ -82,6 +83,8 @@ int ensure_multi_staging(ovl_ctx *c, int nrhs) {
     c->multi_cap = nrhs;
     return OVL_OK;
 }
+
+int set_deflation_strided(ovl_ctx *c, int nev, const void *phi, const double *lambda, size_t vec_stride);
 
 // canonical in -> native psi_n, run `body(psi_n, out_n)`, native out_n -> canonical out
 template <typename F> int with_canonical(ovl_ctx *c, const void *psi, void *out, F body) {
@@ -313,7 +316,14 @@ int ovl_set_graphs(ovl_ctx *c, int on) {
 }
 
 int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda) {
-    if (!c) return OVL_EINVAL;
+    return c ? set_deflation_strided(c, nev, phi, lambda, c->n() * sizeof(double2)) : OVL_EINVAL;
+}
+
+}  // extern "C"
+
+namespace {
+// the deflation space from vectors that start `vec_stride` bytes apart (a slab's part of global eigenvectors)
+int set_deflation_strided(ovl_ctx *c, int nev, const void *phi, const double *lambda, size_t vec_stride) {
     if (nev < 0 || (nev > 0 && (!phi || !lambda))) return fail(c, OVL_EINVAL, "nev >= 0 and non-null phi, lambda are required");
     for (int i = 0; i < nev; ++i)
         if (!std::isfinite(lambda[i]) || std::fabs(lambda[i]) < 1e-14 * c->lambda_max)
@@ -340,7 +350,7 @@ int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda
     const bool dev = is_device_ptr(phi);
     if (!dev) OVL_TRY(dev_alloc(c, &c->stage_in, vb));
     for (int i = 0; i < nev; ++i) {
-        const double2 *src = (const double2 *)((const char *)phi + (size_t)i * vb);
+        const double2 *src = (const double2 *)((const char *)phi + (size_t)i * vec_stride);
         if (!dev) {
             OVL_CUDA(c, cudaMemcpyAsync(c->stage_in, src, vb, cudaMemcpyHostToDevice, c->st));
             src = (const double2 *)c->stage_in;
@@ -353,6 +363,9 @@ int ovl_set_deflation(ovl_ctx *c, int nev, const void *phi, const double *lambda
     c->coef_stale = true;
     return OVL_OK;
 }
+}  // namespace
+
+extern "C" {
 
 int ovl_dw(ovl_ctx *c, const void *psi, void *out) {
     return with_canonical(c, psi, out, [&](const void *i, void *o) { return DISPATCH(c, dw_native, c, i, o); });
@@ -508,5 +521,182 @@ int ovl_poly_timings(ovl_ctx *c, int max_n, float *ms_out, int *n_out) {
     return OVL_OK;
 }
 long long ovl_launch_count(const ovl_ctx *c) { return c ? c->launches : 0; }
+
+
+// ---------------------------------------------------------------------------------------------- t-split lattice (ovl_group)
+
+int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void *links_c128, int prec, int recon,
+                     void *const *cuda_streams, const int *devices) {
+    if (!out) return OVL_EINVAL;
+    *out = nullptr;
+    if (!links_c128 || !cuda_streams || check_cfg(dims, prec, recon) != OVL_OK) return OVL_EINVAL;
+    if (nslabs < 1 || nslabs > MAX_SLABS || dims[3] % nslabs != 0 || dims[3] / nslabs < 2) return OVL_EINVAL;
+    ovl_group *g = new (std::nothrow) ovl_group();
+    if (!g) return OVL_ENOMEM;
+    g->n = nslabs; g->prec = prec; g->recon = recon;
+    for (int i = 0; i < 4; ++i) g->gdims[i] = dims[i];
+    const int ldims[4] = {dims[0], dims[1], dims[2], dims[3] / nslabs};
+    g->Vloc = (size_t)ldims[0] * ldims[1] * ldims[2] * ldims[3];
+    g->w.resize(nslabs);
+    int cur = 0;
+    cudaGetDevice(&cur);
+    for (int r = 0; r < nslabs; ++r) g->dev.push_back(devices ? devices[r] : cur);
+    auto body = [&]() -> int {
+        for (int r = 0; r < nslabs; ++r)  // every slab reads its neighbours' halos and every slab's reduction scratch
+            for (int q = 0; q < nslabs; ++q)
+                if (g->dev[r] != g->dev[q]) {
+                    DevGuard dg(g->dev[r]);
+                    cudaError_t e = cudaDeviceEnablePeerAccess(g->dev[q], 0);
+                    if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled)
+                        return gfail(g, OVL_ECUDA, "no peer access from device %d to %d: %s", g->dev[r], g->dev[q], cudaGetErrorString(e));
+                    cudaGetLastError();
+                }
+        const size_t ts = prec == OVL_F64 ? 8 : 4;
+        for (int r = 0; r < nslabs; ++r) {
+            DevGuard dg(g->dev[r]);
+            ovl_ctx *c = nullptr;
+            const char *lk = (const char *)links_c128 + (size_t)r * g->Vloc * 36 * sizeof(double2);
+            int rc = create_impl(&c, ldims, lk, prec, recon, cuda_streams[r], nullptr, 0, 0, 1, 0);
+            if (rc != OVL_OK) return gfail(g, rc, "slab %d: context creation failed", r);
+            g->s.push_back(c);
+            c->use_graphs = false;  // the launch sequence of a slab is interleaved with event waits on its neighbours
+            const size_t face = (size_t)12 * c->g.sxyz * 2 * ts;
+            for (int sl = 0; sl < 3; ++sl)
+                for (int side = 0; side < 2; ++side) GRP_TRY(g, r, dev_alloc(c, &g->w[r].halo[sl][side], face));
+            GRP_TRY(g, r, dev_alloc(c, &g->w[r].u_lo, (size_t)c->nrow() * 3 * c->g.sxyz * 2 * ts));
+            for (int b = 0; b < 2; ++b) {
+                GRP_TRY(g, r, dev_alloc(c, (void **)&g->w[r].red_loc[b], sizeof(double) * 8));
+                GRP_CUDA(g, cudaEventCreateWithFlags(&g->w[r].ev[b], cudaEventDisableTiming));
+            }
+        }
+        // the backward t hop of a slab's first time slice needs U_t of the lower neighbour's last slice: sent once, here
+        for (int r = 0; r < nslabs; ++r) {
+            const int lo = lo_of(g, r);
+            ovl_ctx *cl = g->s[lo];
+            DevGuard dg(g->dev[lo]);
+            const int npl = cl->nrow() * 3;
+            const size_t ne = (size_t)npl * cl->g.sxyz;
+            if (prec == OVL_F64)
+                k_pack_ut_last<double><<<(unsigned)((ne + 255) / 256), 256, 0, cl->st>>>(
+                    cl->g.V, cl->g.sxyz, npl, (const double2 *)cl->U + (size_t)3 * npl * cl->g.V, (double2 *)g->w[r].u_lo);
+            else
+                k_pack_ut_last<float><<<(unsigned)((ne + 255) / 256), 256, 0, cl->st>>>(
+                    cl->g.V, cl->g.sxyz, npl, (const float2 *)cl->U + (size_t)3 * npl * cl->g.V, (float2 *)g->w[r].u_lo);
+            GRP_CUDA(g, cudaGetLastError());
+        }
+        for (int r = 0; r < nslabs; ++r) {
+            DevGuard dg(g->dev[r]);
+            GRP_CUDA(g, cudaStreamSynchronize(g->s[r]->st));
+        }
+        return OVL_OK;
+    };
+    const int rc = body();
+    if (rc != OVL_OK) { ovl_group_destroy(g); return rc; }
+    *out = g;
+    return OVL_OK;
+}
+
+int ovl_group_destroy(ovl_group *g) {
+    if (!g) return OVL_EINVAL;
+    for (size_t r = 0; r < g->s.size(); ++r) {
+        DevGuard dg(g->dev[r]);
+        cudaStreamSynchronize(g->s[r]->st);
+    }
+    for (size_t r = 0; r < g->s.size(); ++r) {
+        DevGuard dg(g->dev[r]);
+        for (int b = 0; b < 2; ++b)
+            if (g->w[r].ev[b]) cudaEventDestroy(g->w[r].ev[b]);
+        ovl_destroy(g->s[r]);
+    }
+    delete g;
+    return OVL_OK;
+}
+
+int ovl_group_slabs(const ovl_group *g) { return g ? g->n : 0; }
+const char *ovl_group_last_error(const ovl_group *g) { return g ? g->err : "null group"; }
+long long ovl_group_launch_count(const ovl_group *g) {
+    long long t = 0;
+    if (g) for (ovl_ctx *c : g->s) t += c->launches;
+    return t;
+}
+
+int ovl_group_set_kernel(ovl_group *g, double m_w, double lambda_max) {
+    if (!g) return OVL_EINVAL;
+    for (int r = 0; r < g->n; ++r) GRP_TRY(g, r, ovl_set_kernel(g->s[r], m_w, lambda_max));
+    return OVL_OK;
+}
+int ovl_group_set_chebyshev(ovl_group *g, int N, const double *alpha) {
+    if (!g) return OVL_EINVAL;
+    for (int r = 0; r < g->n; ++r) GRP_TRY(g, r, ovl_set_chebyshev(g->s[r], N, alpha));
+    return OVL_OK;
+}
+int ovl_group_set_deflation(ovl_group *g, int nev, const void *phi, const double *lambda) {
+    if (!g) return OVL_EINVAL;
+    const size_t vstride = (size_t)g->n * g->Vloc * 12 * sizeof(double2);  // one GLOBAL eigenvector
+    for (int r = 0; r < g->n; ++r) {
+        DevGuard dg(g->dev[r]);
+        const char *p = phi ? (const char *)phi + (size_t)r * g->Vloc * 12 * sizeof(double2) : nullptr;
+        GRP_TRY(g, r, set_deflation_strided(g->s[r], nev, p, lambda, vstride));
+        if (nev > g->wcap)
+            for (int b = 0; b < 2; ++b) {
+                dev_release(g->s[r], (void **)&g->w[r].w_loc[b]);
+                GRP_TRY(g, r, dev_alloc(g->s[r], (void **)&g->w[r].w_loc[b], sizeof(double2) * nev));
+            }
+    }
+    if (nev > g->wcap) g->wcap = nev;
+    g->nev = nev;
+    return OVL_OK;
+}
+
+}  // extern "C"
+
+namespace {
+// canonical GLOBAL field -> every slab's psi_n, body on the slabs' native fields, every slab's out_n -> canonical GLOBAL field
+template <typename F> int group_with_canonical(ovl_group *g, const void *psi, void *out, F body) {
+    if (!g) return OVL_EINVAL;
+    if (!psi || !out || psi == out) return gfail(g, OVL_EINVAL, "null or aliased spinor pointers");
+    std::vector<void *> in(g->n), o(g->n);
+    for (int r = 0; r < g->n; ++r) {
+        ovl_ctx *c = g->s[r];
+        DevGuard dg(g->dev[r]);
+        GRP_TRY(g, r, import_any(c, (const char *)psi + (size_t)r * c->canon_bytes(), c->psi_n));
+        in[r] = c->psi_n; o[r] = c->out_n;
+    }
+    const int rc = body(in.data(), o.data());
+    if (rc != OVL_OK && rc != OVL_ENOTCONV) return rc;
+    for (int r = 0; r < g->n; ++r) {
+        ovl_ctx *c = g->s[r];
+        DevGuard dg(g->dev[r]);
+        GRP_TRY(g, r, export_any(c, c->out_n, (char *)out + (size_t)r * c->canon_bytes()));
+    }
+    for (int r = 0; r < g->n; ++r) {  // the group calls synchronise: their result spans several streams
+        DevGuard dg(g->dev[r]);
+        GRP_CUDA(g, cudaStreamSynchronize(g->s[r]->st));
+    }
+    return rc;
+}
+#define GDISPATCH(g, fn, ...) ((g)->prec == OVL_F64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
+}  // namespace
+
+extern "C" {
+
+int ovl_group_dw(ovl_group *g, const void *psi, void *out) {
+    return group_with_canonical(g, psi, out, [&](void *const *i, void *const *o) { return GDISPATCH(g, group_stencil, g, 0, i, o); });
+}
+int ovl_group_khat(ovl_group *g, const void *psi, void *out) {
+    return group_with_canonical(g, psi, out, [&](void *const *i, void *const *o) { return GDISPATCH(g, group_stencil, g, 1, i, o); });
+}
+int ovl_group_sign(ovl_group *g, const void *psi, void *out) {
+    return group_with_canonical(g, psi, out, [&](void *const *i, void *const *o) { return GDISPATCH(g, group_sign_combine, g, 0.0, 1.0, 0, 0, i, o); });
+}
+int ovl_group_overlap(ovl_group *g, double mu, int dagger, const void *psi, void *out) {
+    return group_with_canonical(g, psi, out, [&](void *const *i, void *const *o) { return GDISPATCH(g, group_overlap, g, mu, dagger ? 1 : 0, i, o); });
+}
+int ovl_group_cg(ovl_group *g, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out, double *relres_out) {
+    if (!g) return OVL_EINVAL;
+    if (!iters_out || !relres_out || maxiter < 0) return gfail(g, OVL_EINVAL, "bad ovl_group_cg arguments");
+    if (g->s[0]->alpha.empty()) return gfail(g, OVL_ESTATE, "ovl_group_set_chebyshev has not been called");
+    return group_with_canonical(g, b, x, [&](void *const *i, void *const *o) { return GDISPATCH(g, group_cg, g, mu, i, o, tol, maxiter, iters_out, relres_out); });
+}
 
 }  // extern "C"

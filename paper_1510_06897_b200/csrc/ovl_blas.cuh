@@ -288,6 +288,21 @@ __global__ void k_axpy_mixed(size_t n, double scale, const cx<TE> *__restrict__ 
 // second stage of the CG reductions, one block per system (blockIdx.x = rhs).  what: 0 -> bb = rr = sum (start),
 // 1 -> pAp = sum, alpha = rr / pAp (0 if frozen), 2 -> rr_new = sum, beta = rr_new / rr, rr = rr_new; the system is
 // frozen once rr_new <= tol2 * bb (tol2 = 0: never), 3 -> sc[SC_PAP] = sum (generic norm^2 read-out)
+// the scalar recurrences of CG given a freshly reduced sum r (see k_cg_scalars)
+__device__ __forceinline__ void cg_scalar_update(double *sc, double r, int what, double tol2) {
+    const bool frozen = sc[SC_FROZEN] != 0.0;
+    // a zero right-hand side is frozen from the start (x = 0 is its solution; 0/0 must not reach the vectors)
+    if (what == 0) { sc[SC_BB] = r; sc[SC_RR] = r; sc[SC_FROZEN] = r == 0.0 ? 1.0 : 0.0; sc[SC_ALPHA] = 0.0; sc[SC_BETA] = 0.0; }
+    else if (what == 1) { sc[SC_PAP] = r; sc[SC_ALPHA] = (frozen || r == 0.0) ? 0.0 : sc[SC_RR] / r; }
+    else if (what == 2) {
+        if (frozen) sc[SC_BETA] = 0.0;
+        else {
+            sc[SC_BETA] = r / sc[SC_RR];
+            sc[SC_RR] = r;
+            if (tol2 > 0.0 && r <= tol2 * sc[SC_BB]) { sc[SC_FROZEN] = 1.0; sc[SC_BETA] = 0.0; }
+        }
+    } else { sc[SC_PAP] = r; }
+}
 __global__ void __launch_bounds__(BLAS_THREADS)
 k_cg_scalars(int nblk, const double *__restrict__ partial, double *sc, int what, double tol2) {
     __shared__ double sm[BLAS_THREADS / 32];
@@ -296,20 +311,7 @@ k_cg_scalars(int nblk, const double *__restrict__ partial, double *sc, int what,
     double r = 0;
     for (int b = threadIdx.x; b < nblk; b += blockDim.x) r += partial[b];
     r = block_sum(r, sm);
-    if (threadIdx.x == 0) {
-        const bool frozen = sc[SC_FROZEN] != 0.0;
-        // a zero right-hand side is frozen from the start (x = 0 is its solution; 0/0 must not reach the vectors)
-        if (what == 0) { sc[SC_BB] = r; sc[SC_RR] = r; sc[SC_FROZEN] = r == 0.0 ? 1.0 : 0.0; sc[SC_ALPHA] = 0.0; sc[SC_BETA] = 0.0; }
-        else if (what == 1) { sc[SC_PAP] = r; sc[SC_ALPHA] = (frozen || r == 0.0) ? 0.0 : sc[SC_RR] / r; }
-        else if (what == 2) {
-            if (frozen) sc[SC_BETA] = 0.0;
-            else {
-                sc[SC_BETA] = r / sc[SC_RR];
-                sc[SC_RR] = r;
-                if (tol2 > 0.0 && r <= tol2 * sc[SC_BB]) { sc[SC_FROZEN] = 1.0; sc[SC_BETA] = 0.0; }
-            }
-        } else { sc[SC_PAP] = r; }
-    }
+    if (threadIdx.x == 0) cg_scalar_update(sc, r, what, tol2);
 }
 
 }  // namespace ovl
