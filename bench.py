@@ -284,16 +284,18 @@ def dslash_sweep(torch, api, hbm_peak, reps=100):
 
 
 def bench_overlap(torch, api, B, w, prec, recon, steps, warmup, dist, rank, with_e2e, host_inputs=None,
-                  recurrence="clenshaw", keep_output=False):
+                  recurrence="clenshaw", keep_output=False, variant="register"):
     """Resident + end-to-end timing of one workload in one precision. Returns a dict of measurements."""
     U, psi, alpha, phi, lam = host_inputs if host_inputs is not None else make_inputs(w, seed_off=rank)
     dims, mu = w["dims"], w["mu"]
     V = int(np.prod(dims))
     pb = 8 if prec == "f64" else 4
-    op = api.Overlap(dims, torch.from_numpy(U).cuda(), prec, recon)
-    res = {}
+    # the context lives in a torch-owned workspace (ovl_create_ws): no allocation inside any timed call
+    op = api.Overlap(dims, torch.from_numpy(U).cuda(), prec, recon, workspace=dict(max_nev=w["nev"], max_rhs=1))
+    res = {"workspace_bytes": op.workspace_bytes}
     try:
         op.set_recurrence(recurrence)
+        op.set_fused_variant(variant)
         orders = op.set_chebyshev(alpha)
         if w["nev"]:
             phid = torch.from_numpy(phi).cuda()
@@ -388,6 +390,63 @@ def bench_cg(torch, api, w, steps_tol=1e-8):
     return {"workload": "BASELINE config 2: 8^3x32, mu=0.05, CG on D^dagD to 1e-8, 20-vector deflated degree-200 sign",
             "iterations": it, "true_relres": rel, "converged": ok, "seconds": dt, "overlap_applies": applies,
             "applies_per_s": applies / dt, "us_per_order": 1e6 * dt / (applies * orders)}
+
+
+def bench_cg_chiral(torch, api, w, tol=1e-8):
+    """CG in the chirality sector (one sign application per iteration, reading R23) on the config-2
+    system with a chiral source, against the full D^dag D solve of the same projected source."""
+    U, b, alpha, phi, lam = make_inputs(w, seed_off=inputs.CFG2_SEED_OFF)
+    b = b.copy()
+    b[:, 2:] = 0.0  # positive chirality (gamma5 = diag(1,1,-1,-1))
+    with api.Overlap(w["dims"], torch.from_numpy(U).cuda()) as op:
+        orders = op.set_chebyshev(alpha)
+        op.set_deflation(torch.from_numpy(phi).cuda(), lam)
+        bd = torch.from_numpy(b).cuda()
+        op.cg_chiral(bd, inputs.CFG2_MU, +1, tol=0.0, maxiter=1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        x, it, rel, ok = op.cg_chiral(bd, inputs.CFG2_MU, +1, tol=tol, maxiter=2000)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        xf, itf, relf, okf = op.cg(bd, inputs.CFG2_MU, tol=tol, maxiter=2000)
+        torch.cuda.synchronize()
+        dtf = time.perf_counter() - t0
+        diff = float(torch.linalg.norm(x - xf) / torch.linalg.norm(xf))
+    return {"chiral_seconds": dt, "chiral_iterations": it, "chiral_true_relres": rel, "converged": ok, "full_seconds": dtf,
+            "full_iterations": itf, "speedup": dtf / dt, "rel_diff_of_solutions": diff, "sign_applies_per_iteration": 1}
+
+
+def bench_split(torch, api, w, host_inputs, nslabs_list=(2, 4), steps=3):
+    """SURVEY §8(f) rank 3 on ONE GPU: the lattice split along t into slabs that run in their own streams with the halo
+    stores fused into the stencil kernel.  On one GPU the slabs only share the device, so this measures the overhead of the
+    decomposition (event ordering, direct launches, halo stores), not a speed-up; results are checked bit for bit against the
+    undivided operator (no deflation: reductions are partitioned differently)."""
+    U, psi, alpha, phi, lam = host_inputs
+    Ud = torch.from_numpy(U).cuda()
+    p = torch.from_numpy(psi).cuda()
+    out = {}
+    with api.Overlap(w["dims"], Ud) as ref:
+        ref.set_chebyshev(alpha)
+        want = ref.overlap(p, w["mu"])
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            ref.overlap(p, w["mu"])
+        torch.cuda.synchronize()
+        out["undivided_applies_per_s_canonical_io"] = steps / (time.perf_counter() - t0)
+    for ns in nslabs_list:
+        with api.SplitOverlap(w["dims"], Ud, ns) as sp:
+            sp.set_chebyshev(alpha)
+            got = sp.overlap(p, w["mu"])
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(steps):
+                sp.overlap(p, w["mu"])
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            out[f"{ns}_slabs"] = {"applies_per_s": steps / dt, "bit_identical_to_undivided": bool(torch.equal(got, want))}
+    return out
 
 
 def bench_cg_multi(torch, api, w, nrhs=12, tol=1e-8):
@@ -501,7 +560,8 @@ def run_native(args, w):
                      "algorithmic_bytes_per_site_per_launch": main["bytes_per_site_per_order"],
                      "frac_of_nominal_8TBs": main["achieved_gbs"] / 8000.0},
     }
-    extras = {"finite": main["finite"], "e2e_bit_identical_to_resident": main.get("e2e_matches_resident")}
+    extras = {"finite": main["finite"], "e2e_bit_identical_to_resident": main.get("e2e_matches_resident"),
+              "workspace_bytes_torch_owned": main["workspace_bytes"]}
     if rank == 0 and n == 1 and not args.no_extras:
         if args.workload == "cfg3":
             w1 = dict(WORKLOADS["cfg1"], name="cfg1")
@@ -512,6 +572,8 @@ def run_native(args, w):
             extras["cfg1_eigensolver"] = bench_eigensolver(torch, api, w1, 20, 40, 200)
             if args.cfg3_eigensolver:  # ~40 s: the 50 pairs of config 3 (block 104 reaches past the 24 + 72 clusters)
                 extras["cfg3_eigensolver"] = bench_eigensolver(torch, api, w, 50, 104, 200)
+            extras["cfg2_cg_chiral"] = bench_cg_chiral(torch, api, w1)
+            extras["tsplit_on_one_gpu_20x20x20x64_no_deflation"] = bench_split(torch, api, w, host_inputs)
             extras["cfg2_cg_12rhs"] = bench_cg_multi(torch, api, w1)
             extras["cfg2_cg_mixed"] = bench_cg_mixed(torch, api, w1, label="config 2 (8^3x32, mu=0.05, tol 1e-8)")
             extras["cfg3_cg_mixed"] = bench_cg_mixed(torch, api, w, host_inputs,
@@ -529,6 +591,12 @@ def run_native(args, w):
                 extras["cfg3_12real_links"] = {"applies_per_s": r12["applies_per_s"], "achieved_gbs": r12["achieved_gbs"],
                                                "frac": r12["achieved_gbs"] / hbm_peak, "kernel_us": r12["kernel_us"],
                                                "algorithmic_bytes_per_site_per_launch": r12["bytes_per_site_per_order"]}
+            rb = bench_overlap(torch, api, B, w, args.prec, args.recon, args.steps, args.warmup, None, 0, False, host_inputs,
+                               args.recurrence, variant="bulk")
+            extras["cfg3_bulk_copy_variant"] = {
+                "what": "OVL_FUSED_BULK: persistent warps, links landed in shared memory by cp.async.bulk + mbarrier (not the default)",
+                "applies_per_s": rb["applies_per_s"], "achieved_gbs": rb["achieved_gbs"], "frac": rb["achieved_gbs"] / hbm_peak,
+                "kernel_us": rb["kernel_us"]}
             other = "forward" if args.recurrence == "clenshaw" else "clenshaw"
             ro = bench_overlap(torch, api, B, w, args.prec, args.recon, args.steps, args.warmup, None, 0, False, host_inputs, other)
             extras[f"cfg3_{other}_recurrence"] = {

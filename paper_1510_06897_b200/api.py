@@ -74,6 +74,11 @@ class Overlap:
         m = {"clenshaw": B.OVL_REC_CLENSHAW, "forward": B.OVL_REC_FORWARD}.get(mode, mode)
         B.ovl_set_recurrence(self.ctx, m)
 
+    def set_fused_variant(self, variant):
+        """'register' (default) or 'bulk' (cp.async.bulk landing zone for the links): same results, see include/ovl.h."""
+        v = {"register": B.OVL_FUSED_REGISTER, "bulk": B.OVL_FUSED_BULK}.get(variant, variant)
+        B.ovl_set_fused_variant(self.ctx, v)
+
     def set_graphs(self, on=True):
         """CUDA-graph replay of the polynomial loop (only effective when the context runs on a non-default stream)."""
         B.ovl_set_graphs(self.ctx, on)

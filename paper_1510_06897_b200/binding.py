@@ -15,6 +15,7 @@ OVL_OK, OVL_EINVAL, OVL_ENOMEM, OVL_ECUDA, OVL_ESTATE, OVL_ENOTCONV = range(6)
 OVL_F64, OVL_F32 = 0, 1
 OVL_RECON18, OVL_RECON12 = 18, 12
 OVL_REC_CLENSHAW, OVL_REC_FORWARD = 0, 1
+OVL_FUSED_REGISTER, OVL_FUSED_BULK = 0, 1
 OVL_MAX_RHS = 12
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -35,6 +36,7 @@ SIGNATURES = {
     "ovl_set_recurrence": (_I, [_P, _I]),
     "ovl_get_recurrence": (_I, [_P]),
     "ovl_set_graphs": (_I, [_P, _I]),
+    "ovl_set_fused_variant": (_I, [_P, _I]),
     "ovl_set_deflation": (_I, [_P, _I, _P, C.POINTER(_D)]),
     "ovl_dw": (_I, [_P, _P, _P]),
     "ovl_khat": (_I, [_P, _P, _P]),
@@ -180,6 +182,10 @@ def ovl_set_recurrence(ctx, mode):
 
 def ovl_get_recurrence(ctx) -> int:
     return int(load_library().ovl_get_recurrence(ctx))
+
+
+def ovl_set_fused_variant(ctx, variant):
+    return _check(ctx, load_library().ovl_set_fused_variant(ctx, int(variant)))
 
 
 def ovl_set_graphs(ctx, on=True):

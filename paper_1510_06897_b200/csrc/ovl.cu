@@ -137,6 +137,11 @@ int create_impl(ovl_ctx **out, const int dims[4], const void *links_c128, int pr
     c->prec = prec;
     c->recon = recon;
     c->st = (cudaStream_t)cuda_stream;
+    {
+        int dv = 0, sms = 0;
+        if (cudaGetDevice(&dv) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dv) == cudaSuccess && sms > 0) c->sm_count = sms;
+        cudaGetLastError();
+    }
     c->red_nblk = grid_for(c->n(), BLAS_THREADS * 4, 148 * 8);
     c->proj_nblk = (int)((c->n() + BLAS_THREADS * PROJ_EPT - 1) / (BLAS_THREADS * PROJ_EPT));
     auto body = [&]() -> int {
@@ -308,6 +313,14 @@ int ovl_set_recurrence(ovl_ctx *c, int mode) {
     return OVL_OK;
 }
 int ovl_get_recurrence(const ovl_ctx *c) { return c ? c->recurrence : -1; }
+
+int ovl_set_fused_variant(ovl_ctx *c, int variant) {
+    if (!c) return OVL_EINVAL;
+    if (variant != OVL_FUSED_REGISTER && variant != OVL_FUSED_BULK) return fail(c, OVL_EINVAL, "unknown fused-kernel variant %d", variant);
+    c->fused_variant = variant;
+    ++c->poly_gen;  // captured graphs hold the other kernel
+    return OVL_OK;
+}
 
 int ovl_set_graphs(ovl_ctx *c, int on) {
     if (!c) return OVL_EINVAL;

@@ -13,7 +13,8 @@
 
 struct ovl_ctx {
     ovl::Geom g{};
-    int prec = OVL_F64, recon = OVL_RECON18, recurrence = OVL_REC_CLENSHAW;
+    int prec = OVL_F64, recon = OVL_RECON18, recurrence = OVL_REC_CLENSHAW, fused_variant = OVL_FUSED_REGISTER;
+    int sm_count = 148;
     cudaStream_t st = nullptr;
     double m_w = 1.5, lambda_max = 6.5;
 

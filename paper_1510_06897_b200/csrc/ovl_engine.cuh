@@ -4,6 +4,7 @@
 #include "ovl_blas.cuh"
 #include "ovl_ctx.cuh"
 #include "ovl_wilson.cuh"
+#include "ovl_wilson_tp.cuh"
 
 namespace ovl {
 
@@ -27,10 +28,36 @@ struct WilsonArgs {
     int flip = 0, nrhs = 1;
 };
 
+// The bulk-copy variant (ovl_wilson_tp.cuh; ovl_set_fused_variant): persistent warps, the warp's own links landed in shared
+// memory by cp.async.bulk + mbarrier.  4 warps per CTA; 2 (fp64) / 4 (fp32) CTAs per SM keep 147 KB of landing zone and
+// leave 81 KB of L1 for the neighbour reuse -- the best staged configuration measured on B200, and still
+// slower than the register-landing kernel, which therefore stays the default.
+template <typename T, int RECON, int FLAGS> inline void launch_wilson_tp(ovl_ctx *c, const WilsonArgs &a, const StepParams<T> &sp) {
+    constexpr int NW = 4, MINB = sizeof(T) == 8 ? 2 : 4, OPT = STG_LINKS;
+    using SM = TpSmem<T, RECON, FLAGS, OPT>;
+    auto kern = k_wilson_tp<T, RECON, FLAGS, OPT, NW, MINB>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::total(NW));
+        attr_set = true;
+    }
+    const int nsub = c->g.V / 32;
+    int grid = c->sm_count * MINB;
+    if (grid * NW > nsub) grid = (nsub + NW - 1) / NW;
+    kern<<<grid, NW * 32, SM::total(NW), c->st>>>(c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi,
+                                                  (cx<T> *)a.out, sp, nsub);
+}
+
 template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx *c, const WilsonArgs &a) {
     constexpr int TH = WilsonCfg<T>::THREADS;
     const int grid = ((c->g.V + TH - 1) / TH) * a.nrhs;
     StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip};
+    if constexpr (!(FLAGS & (K_ACC | K_ACCI | K_NOWRITE))) {
+        if (c->fused_variant == OVL_FUSED_BULK && a.nrhs == 1 && c->g.V % 32 == 0 && c->g.sxyz % 32 == 0) {
+            launch_wilson_tp<T, RECON, FLAGS>(c, a, sp);
+            return;
+        }
+    }
     if (a.nrhs > 1)
         k_wilson_fused_multi<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
             c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp,

@@ -157,3 +157,20 @@ def test_config3_true_eigenpairs_degree400_nev50_full_size(torch, api, prec, tol
     assert rel_err(got, want) < tol
     for i, ei in zip((0, 49), e):
         assert rel_err(ei, np.sign(lam[i]) * phi[i]) < (1e-12 if prec == "f64" else tol)
+
+
+@pytest.mark.parametrize("nslabs", [2, 4])
+def test_split_lattice_full_size_bit_identical(torch, api, rough, nslabs):
+    """SURVEY §8(f) rank 3 at 20^3 x 64: the lattice split along t into 2 and 4 slabs (32 / 16 time slices each, 250 / 125
+    tiles per slab), halo stores fused into the stencil kernel: D_W and a degree-21 polynomial sign function bit-identical
+    to the undivided lattice (which the tests above hold against the oracle)."""
+    U, psi = rough
+    alpha = inputs.chebyshev_sign_coeffs(21, 0.3)
+    Ud = dev(torch, U)
+    with api.Overlap(DIMS, Ud) as ref, api.SplitOverlap(DIMS, Ud, nslabs) as sp:
+        p = dev(torch, psi)
+        for o in (ref, sp):
+            o.set_chebyshev(alpha)
+        assert torch.equal(sp.dw(p), ref.dw(p))
+        assert torch.equal(sp.sign(p), ref.sign(p))
+        assert torch.equal(sp.overlap(p, 0.01, dagger=True), ref.overlap(p, 0.01, dagger=True))

@@ -790,3 +790,31 @@ def test_cg_chiral_argument_checks(torch, api):
         z[:, 2:] = b[:, 2:]                                                  # purely negative chirality
         x0, it0, rel0, ok0 = op.cg_chiral(z, 0.1, +1, tol=1e-9, maxiter=10)
         assert ok0 and it0 == 0 and rel0 == 0.0 and torch.count_nonzero(x0).item() == 0
+
+
+@pytest.mark.parametrize("prec,recon", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 32), (4, 4, 4, 6), (6, 6, 6, 8)])
+def test_bulk_copy_variant_bit_identical(torch, api, orc, prec, recon, dims):
+    """OVL_FUSED_BULK (persistent warps, the links landed in shared memory by cp.async.bulk + mbarrier) gives the same bits
+    as the default register-landing kernel: D_W, K^, the deflated sign function (both eligible and fallback lattices:
+    6^3 x 8 has Lx Ly Lz = 216, not a multiple of 32, and silently stays on the default kernel)."""
+    U = inputs.config_links(dims, 0.4, 51, stout_steps=1)
+    psi = inputs.gaussian_spinor(dims, 52)
+    alpha = rough_alpha(24, seed=7)
+    phi = inputs.orthonormal_vectors(dims, 2, 53)
+    lam = np.array([0.5, -0.6])
+    with api.Overlap(dims, dev(torch, U), prec, recon) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        p = dev(torch, psi, op.cdtype)
+        want = [op.dw(p), op.khat(p), op.sign(p), op.overlap(p, 0.1, dagger=True)]
+        op.set_fused_variant("bulk")
+        got = [op.dw(p), op.khat(p), op.sign(p), op.overlap(p, 0.1, dagger=True)]
+        again = op.sign(p)
+        op.set_fused_variant("register")
+        back = op.sign(p)
+    for g_, w_ in zip(got, want):
+        assert torch.equal(g_, w_)
+    assert torch.equal(again, want[2]) and torch.equal(back, want[2])
+    tol = TOL_OVL if prec == "f64" else TOL_F32
+    assert rel_err(host(got[2]).astype(np.complex128), orc.sign(dims, U, alpha, psi, phi, lam)) < tol
