@@ -64,11 +64,12 @@ __device__ __forceinline__ void load_link(cx<T> (&u)[3][3], const cx<T> *__restr
     }
 }
 
-// The arithmetic of one hop given the neighbour spinor p and the link u (already in registers): spin projection to a half
-// spinor, 3x3 colour multiply (U for FWD = 1, U^dag for FWD = 0), reconstruction into the 12 accumulators.
+// The arithmetic of one hop given the neighbour spinor p and the link u (already in registers), in two halves:
+//   hop_half   spin projection to a half spinor and the 3x3 colour multiply (U for FWD = 1, U^dag for FWD = 0): g0, g1;
+//   hop_accum  reconstruction of the four spin rows from (g0, g1), added to the 12 accumulators (one addition each).
 // MU direction, FWD = 1: (1 - gamma_mu) U_mu(x) in(x+mu);  FWD = 0: (1 + gamma_mu) U_mu(x-mu)^dag in(x-mu); bs = boundary phase.
 template <typename T, int MU, int FWD>
-__device__ __forceinline__ void hop_math(cx<T> (&hop)[12], const cx<T> (&p)[12], const cx<T> (&u)[3][3], T bs) {
+__device__ __forceinline__ void hop_half(cx<T> (&g0)[3], cx<T> (&g1)[3], const cx<T> (&p)[12], const cx<T> (&u)[3][3], T bs) {
     cx<T> h0[3], h1[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -91,7 +92,6 @@ __device__ __forceinline__ void hop_math(cx<T> (&hop)[12], const cx<T> (&p)[12],
             h1[c].x *= bs; h1[c].y *= bs;
         }
     }
-    cx<T> g0[3], g1[3];
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         g0[i] = mk<T>(0, 0);
@@ -107,25 +107,42 @@ __device__ __forceinline__ void hop_math(cx<T> (&hop)[12], const cx<T> (&p)[12],
             }
         }
     }
+}
+// row r (0..3) of the reconstructed hop for colour c, added to acc:  rows 0, 1 are g0, g1; rows 2, 3 follow the table in the
+// file header (s = -1 for FWD, +1 for backward)
+template <typename T, int MU, int FWD, int ROW>
+__device__ __forceinline__ cx<T> hop_row_add(cx<T> acc, cx<T> g0c, cx<T> g1c) {
+    if (ROW == 0) return cadd(acc, g0c);
+    if (ROW == 1) return cadd(acc, g1c);
+    if (MU == 0) {  // r2 = -s i h1, r3 = -s i h0
+        if (ROW == 2) return FWD ? caddi(acc, g1c) : csubi(acc, g1c);
+        return FWD ? caddi(acc, g0c) : csubi(acc, g0c);
+    } else if (MU == 1) {  // r2 = s h1, r3 = -s h0
+        if (ROW == 2) return FWD ? csub(acc, g1c) : cadd(acc, g1c);
+        return FWD ? cadd(acc, g0c) : csub(acc, g0c);
+    } else if (MU == 2) {  // r2 = -s i h0, r3 = s i h1
+        if (ROW == 2) return FWD ? caddi(acc, g0c) : csubi(acc, g0c);
+        return FWD ? csubi(acc, g1c) : caddi(acc, g1c);
+    } else {  // r2 = s h0, r3 = s h1
+        if (ROW == 2) return FWD ? csub(acc, g0c) : cadd(acc, g0c);
+        return FWD ? csub(acc, g1c) : cadd(acc, g1c);
+    }
+}
+template <typename T, int MU, int FWD>
+__device__ __forceinline__ void hop_accum(cx<T> (&hop)[12], const cx<T> (&g0)[3], const cx<T> (&g1)[3]) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        hop[c] = cadd(hop[c], g0[c]);
-        hop[3 + c] = cadd(hop[3 + c], g1[c]);
-        // s = -1 for FWD, +1 for backward
-        if (MU == 0) {  // r2 = -s i h1, r3 = -s i h0
-            hop[6 + c] = FWD ? caddi(hop[6 + c], g1[c]) : csubi(hop[6 + c], g1[c]);
-            hop[9 + c] = FWD ? caddi(hop[9 + c], g0[c]) : csubi(hop[9 + c], g0[c]);
-        } else if (MU == 1) {  // r2 = s h1, r3 = -s h0
-            hop[6 + c] = FWD ? csub(hop[6 + c], g1[c]) : cadd(hop[6 + c], g1[c]);
-            hop[9 + c] = FWD ? cadd(hop[9 + c], g0[c]) : csub(hop[9 + c], g0[c]);
-        } else if (MU == 2) {  // r2 = -s i h0, r3 = s i h1
-            hop[6 + c] = FWD ? caddi(hop[6 + c], g0[c]) : csubi(hop[6 + c], g0[c]);
-            hop[9 + c] = FWD ? csubi(hop[9 + c], g1[c]) : caddi(hop[9 + c], g1[c]);
-        } else {  // r2 = s h0, r3 = s h1
-            hop[6 + c] = FWD ? csub(hop[6 + c], g0[c]) : cadd(hop[6 + c], g0[c]);
-            hop[9 + c] = FWD ? csub(hop[9 + c], g1[c]) : cadd(hop[9 + c], g1[c]);
-        }
+        hop[c] = hop_row_add<T, MU, FWD, 0>(hop[c], g0[c], g1[c]);
+        hop[3 + c] = hop_row_add<T, MU, FWD, 1>(hop[3 + c], g0[c], g1[c]);
+        hop[6 + c] = hop_row_add<T, MU, FWD, 2>(hop[6 + c], g0[c], g1[c]);
+        hop[9 + c] = hop_row_add<T, MU, FWD, 3>(hop[9 + c], g0[c], g1[c]);
     }
+}
+template <typename T, int MU, int FWD>
+__device__ __forceinline__ void hop_math(cx<T> (&hop)[12], const cx<T> (&p)[12], const cx<T> (&u)[3][3], T bs) {
+    cx<T> g0[3], g1[3];
+    hop_half<T, MU, FWD>(g0, g1, p, u, bs);
+    hop_accum<T, MU, FWD>(hop, g0, g1);
 }
 
 // One hop with both operands loaded from global memory: sn = neighbour site, su = site that owns the link.
