@@ -508,6 +508,36 @@ def bench_eigensolver(torch, api, w, nev, block, degree):
             "max_residual": float(res.max()), "abs_lambda_min": float(np.abs(lam).min()), "abs_lambda_max": float(np.abs(lam).max())}
 
 
+def run_profile_target(args, w):
+    """Short single-purpose runs for ncu captures (profiles/): no JSON line, no timing claims."""
+    import torch
+
+    from paper_1510_06897_b200 import api, binding as B, build
+    if build.needs_build():
+        build.build_library()
+    B.load_library()
+    st = torch.cuda.Stream()
+    torch.cuda.set_stream(st)
+    if args.profile_target.startswith("multi"):
+        nrhs = int(args.profile_target[5:])
+        U, psi, alpha, phi, lam = make_inputs(w)
+        r = bench_multi(torch, api, w, args.prec, args.recon, nrhs, 1, 1, (U, psi, alpha[:41], phi[:4], lam[:4]))
+        print("profile target", args.profile_target, r)
+    elif args.profile_target == "dw48":
+        dims, block = (48, 48, 48, 96), (12, 12, 12, 24)
+        U = inputs.tiled_links(dims, block, 0.3, inputs.SEED_BASE + 4)
+        psi = inputs.gaussian_spinor(dims, inputs.SEED_BASE + 104)
+        with api.Overlap(dims, U, args.prec, args.recon) as op:
+            p = torch.from_numpy(psi).cuda().to(op.cdtype)
+            a, b = op.to_native(p), op.native_empty()
+            for _ in range(8):
+                op.dw_native(a, b)
+            torch.cuda.synchronize()
+        print("profile target dw48 done")
+    else:
+        raise SystemExit("unknown --profile-target")
+
+
 def run_native(args, w):
     import torch
 
@@ -638,6 +668,7 @@ def main():
     ap.add_argument("--ref-budget-s", type=float, default=330.0,
                     help="--impl reference: stop timing full oracle applies once the next one would pass this many seconds")
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--profile-target", default="", help="ncu captures only: multi4 | multi12 (degree-40 multi-rhs apply) | dw48 (D_W at 48^3x96)")
     ap.add_argument("--cfg3-eigensolver", action="store_true",
                     help="extras: also compute the 50 deflation pairs of config 3 on the GPU (ovl_lowest_eigenpairs, ~40 s)")
     ap.add_argument("--fast-inputs", action="store_true",
@@ -658,7 +689,9 @@ def main():
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
                "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
         raise SystemExit(subprocess.call(cmd))
-    if args.impl == "reference":
+    if args.profile_target:
+        run_profile_target(args, w)
+    elif args.impl == "reference":
         run_reference(args, w)
     else:
         run_native(args, w)
