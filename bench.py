@@ -33,13 +33,17 @@ from paper_1510_06897_b200 import inputs, replicas  # noqa: E402
 WORKLOADS = inputs.WORKLOADS
 
 
+FUSED_KERNEL_SOURCES = ("ovl_wilson.cuh", "ovl_types.cuh", "ovl_engine.cuh")  # body, loads / complex helpers, launch shape
+
+
 def csrc_hash():
-    """sha256 over the kernel sources and the boundary header: the key an ncu capture under profiles/ is valid for."""
+    """sha256 over the sources that define the dominant (fused Wilson/Chebyshev) kernel and its launch configuration:
+    the key an ncu capture under profiles/ is valid for."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_1510_06897_b200", "csrc")
-    for f in sorted(os.listdir(d)) + [os.path.join(ROOT, "include", "ovl.h")]:
-        with open(os.path.join(d, f) if not os.path.isabs(f) else f, "rb") as fh:
+    for f in FUSED_KERNEL_SOURCES:
+        with open(os.path.join(d, f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
 
