@@ -542,6 +542,55 @@ def run_profile_target(args, w):
         raise SystemExit("unknown --profile-target")
 
 
+def run_tsplit(args, w):
+    """--parallelism tsplit: ONE lattice split along t over the N GPUs of the node (ovl_group_*: one slab per GPU, halo stores
+    fused into the stencil kernel as NVLink peer stores, event-ordered).  The group lives in one process, so under torchrun
+    rank 0 drives all N devices and the other ranks leave at once.  "scaling": "strong" (the lattice is fixed).  Canonical
+    fields in, canonical fields out (device resident); no deflation vectors are timed here -- the split context's timing
+    hooks cover whole applies only."""
+    import torch
+
+    from paper_1510_06897_b200 import api, binding as B, build
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    if build.needs_build():
+        build.build_library()
+    B.load_library()
+    n = args.gpus
+    ndev = torch.cuda.device_count()
+    devices = list(range(n)) if ndev >= n else [0] * n   # fewer GPUs than slabs: several slabs share a device (test mode)
+    torch.cuda.set_device(devices[0])
+    U, psi, alpha, phi, lam = make_inputs(w)
+    Ud = torch.from_numpy(U).cuda()
+    p = torch.from_numpy(psi).cuda()
+    with api.SplitOverlap(w["dims"], Ud, n, args.prec, args.recon, devices=devices if ndev >= n else None) as sp:
+        sp.set_chebyshev(alpha)
+        sp.set_deflation(torch.from_numpy(phi).cuda(), lam)
+        for _ in range(args.warmup):
+            y = sp.overlap(p, w["mu"])
+        torch.cuda.synchronize()
+        sampler = ClockSampler(devices[0]).start()
+        l0 = sp.launch_count()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            y = sp.overlap(p, w["mu"])   # synchronises every slab stream before returning
+        dt = time.perf_counter() - t0
+        clocks = sampler.stop()
+        launches = sp.launch_count() - l0
+    val = args.steps / dt
+    line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": n, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": args.prec, "data": "synthetic",
+            "config": {"workload": w["desc"], "precision": args.prec, "links": f"{args.recon}-real",
+                       "parallelism": f"tsplit x{n} (one lattice, {n} slabs along t" + (")" if ndev >= n else f", all on {ndev} GPU(s): test mode)"),
+                       "timing": "host clock around calls that synchronise all slab streams (canonical device-resident fields in and out)"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                    "note": "device-resident canonical fields; the replicas arm carries the host-buffer e2e number"}}
+    print(json.dumps(line))
+
+
 def run_native(args, w):
     import torch
 
@@ -614,6 +663,7 @@ def run_native(args, w):
                                                      label="config-3 lattice (20^3x64, N=400, 50 vectors), mu=0.05, tol 1e-8")
             extras["multi_rhs"] = {
                 "cfg3_20x20x20x64_fp64_4rhs": bench_multi(torch, api, w, "f64", args.recon, 4, 2, 2, host_inputs),
+                "cfg3_20x20x20x64_fp64_12rhs": bench_multi(torch, api, w, "f64", args.recon, 12, 2, 1, host_inputs),
                 "cfg1_8x8x8x32_fp64_12rhs": bench_multi(torch, api, w1, "f64", 18, 12, 10, 3)}
             if args.prec == "f64":
                 r32 = bench_overlap(torch, api, B, w, "f32", args.recon, args.steps, args.warmup, None, 0, False, host_inputs,
@@ -671,6 +721,8 @@ def main():
                     help="evaluation order of the polynomial sum of eq. 2.3 (ovl_set_recurrence)")
     ap.add_argument("--ref-budget-s", type=float, default=330.0,
                     help="--impl reference: stop timing full oracle applies once the next one would pass this many seconds")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "tsplit"],
+                    help="N > 1: independent replicas (default, weak scaling) or one lattice split along t over the N GPUs")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--profile-target", default="", help="ncu captures only: multi4 | multi12 (degree-40 multi-rhs apply) | dw48 (D_W at 48^3x96)")
     ap.add_argument("--cfg3-eigensolver", action="store_true",
@@ -683,7 +735,7 @@ def main():
     if args.fast_inputs:
         w["stout"] = 0
         w["desc"] += " [--fast-inputs: links NOT smeared; profiling run]"
-    if args.gpus > 1 and "RANK" not in os.environ:
+    if args.gpus > 1 and "RANK" not in os.environ and args.parallelism == "replicas":
         # not under torchrun: launch the N ranks ourselves (one process per GPU, NCCL over 127.0.0.1)
         import socket
         import subprocess
@@ -697,6 +749,8 @@ def main():
         run_profile_target(args, w)
     elif args.impl == "reference":
         run_reference(args, w)
+    elif args.parallelism == "tsplit":
+        run_tsplit(args, w)
     else:
         run_native(args, w)
 

@@ -134,6 +134,17 @@ int create_impl(ovl_ctx **out, const int dims[4], const void *links_c128, int pr
     c->g.V = dims[0] * dims[1] * dims[2] * dims[3];
     c->g.sxy = dims[0] * dims[1];
     c->g.sxyz = c->g.sxy * dims[2];
+    {   // L2-aware sweep (ovl_types.cuh): only when two time slices of a spinor plus one of the links no longer fit half the
+        // L2 (48^3 x 96 class), and only when z-slabs of whole 128-site tiles exist
+        const size_t ts = prec == OVL_F64 ? 8 : 4;
+        const size_t slice_bytes = (size_t)c->g.sxyz * (2 * 24 + 4 * (size_t)(recon == OVL_RECON18 ? 18 : 12)) * ts;
+        if (slice_bytes > (size_t)40 << 20) {
+            int best = 0;
+            for (int zw = 1; zw <= dims[2]; ++zw)
+                if (dims[2] % zw == 0 && ((size_t)c->g.sxy * zw) % 128 == 0 && (size_t)c->g.sxy * zw <= 32768) best = zw;
+            if (best > 0 && best < dims[2]) { c->sweep.tpc = c->g.sxy * best / 128; c->sweep.nzs = dims[2] / best; }
+        }
+    }
     c->prec = prec;
     c->recon = recon;
     c->st = (cudaStream_t)cuda_stream;

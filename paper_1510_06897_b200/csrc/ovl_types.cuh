@@ -46,6 +46,16 @@ struct Geom {
     int V;         // sites
     int sxy, sxyz; // Lx*Ly, Lx*Ly*Lz
 };
+// L2-aware sweep order for lattices whose time slices outgrow the L2: the 128-site tiles are visited z-slab by z-slab
+// (nzs slabs of tpc tiles per time slice), all time slices of a slab before the next slab, so the reuse distance of the t
+// neighbours and of U_t(x - t^) is one slab of one time slice instead of a whole time slice.  Position in the sweep -> tile
+// (a permutation of whole tiles).
+struct Sweep { int tpc, nzs; };
+__device__ __forceinline__ int sweep_tile(const Sweep &sw, int Lt, int pos) {
+    const int c = pos / sw.tpc, w = pos - c * sw.tpc;
+    const int zs = c / Lt, t = c - zs * Lt;
+    return (t * sw.nzs + zs) * sw.tpc + w;
+}
 
 // read-only (non-coherent) loads, for the fields a kernel never writes (links, the stencil operand, psi, eigenvectors);
 // `prev` of the fused kernel may alias its output and is NOT read through this path

@@ -267,6 +267,17 @@ k_wilson_fused(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restric
     wilson_tile<T, RECON, FLAGS, THREADS>(g, U, in, prev, psi, out, acc, sp, tile);
 }
 
+// The same kernel visiting the tiles in the L2-aware z-slab order (Sweep, ovl_types.cuh).  A kernel of its own with its own
+// parameter list: the register allocation of the plain-order kernel at the 168-register cap is fragile, and it stays
+// exactly as it was.
+template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_wilson_fused_swept(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *prev,
+                     const cx<T> *__restrict__ psi, cx<T> *out, cx<T> *__restrict__ acc, const StepParams<T> sp, const Sweep sw) {
+    const int tile = sweep_tile(sw, g.L[3], sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x);
+    wilson_tile<T, RECON, FLAGS, THREADS>(g, U, in, prev, psi, out, acc, sp, tile);
+}
+
 // Several right-hand sides: blockIdx.x = rhs + nrhs * tile, so the CTAs that work on the same
 // tile for different right-hand sides are adjacent in launch order, run at the same time, and the tile's links come from
 // DRAM once and from L2 after that.  Field r starts r * fstride complex elements after field 0.
