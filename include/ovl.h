@@ -230,6 +230,11 @@ int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void 
                      void *const *cuda_streams, const int *devices);
 int ovl_group_destroy(ovl_group *g);
 int ovl_group_slabs(const ovl_group *g);
+/* Split every stencil round of a slab into a boundary launch (its first and last time slice: every halo read and every
+ * push to the neighbours) and an interior launch, with the round's event recorded in between: the neighbours' next round
+ * then overlaps this slab's interior, which hides the cross-GPU event latency.  Same results bit for bit.  Default: on
+ * when the slabs sit on different devices, off when they share one. */
+int ovl_group_set_split_launch(ovl_group *g, int on);
 int ovl_group_set_kernel(ovl_group *g, double m_w, double lambda_max);
 int ovl_group_set_chebyshev(ovl_group *g, int degree_N, const double *alpha);
 int ovl_group_set_deflation(ovl_group *g, int nev, const void *phi_c128, const double *lambda);

@@ -230,6 +230,10 @@ class SplitOverlap:
     def __exit__(self, *a):
         self.close()
 
+    def set_split_launch(self, on=True):
+        """Boundary launch + interior launch per stencil round (hides the cross-GPU event latency); same bits."""
+        B.ovl_group_set_split_launch(self.grp, on)
+
     def set_chebyshev(self, alpha):
         B.ovl_group_set_chebyshev(self.grp, alpha)
 

@@ -52,6 +52,7 @@ SIGNATURES = {
     "ovl_group_create": (_I, [C.POINTER(_P), C.POINTER(_I), _I, _P, _I, _I, C.POINTER(_P), C.POINTER(_I)]),
     "ovl_group_destroy": (_I, [_P]),
     "ovl_group_slabs": (_I, [_P]),
+    "ovl_group_set_split_launch": (_I, [_P, _I]),
     "ovl_group_set_kernel": (_I, [_P, _D, _D]),
     "ovl_group_set_chebyshev": (_I, [_P, _I, C.POINTER(_D)]),
     "ovl_group_set_deflation": (_I, [_P, _I, _P, C.POINTER(_D)]),
@@ -334,6 +335,10 @@ def ovl_group_destroy(g):
 
 def ovl_group_slabs(g) -> int:
     return int(load_library().ovl_group_slabs(g))
+
+
+def ovl_group_set_split_launch(g, on=True):
+    return _gcheck(g, load_library().ovl_group_set_split_launch(g, int(bool(on))))
 
 
 def ovl_group_set_kernel(g, m_w=1.5, lambda_max=6.5):

@@ -565,6 +565,8 @@ int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void 
     int cur = 0;
     cudaGetDevice(&cur);
     for (int r = 0; r < nslabs; ++r) g->dev.push_back(devices ? devices[r] : cur);
+    for (int r = 1; r < nslabs; ++r)
+        if (g->dev[r] != g->dev[0]) g->split_launch = true;
     auto body = [&]() -> int {
         for (int r = 0; r < nslabs; ++r)  // every slab reads its neighbours' halos and every slab's reduction scratch
             for (int q = 0; q < nslabs; ++q)
@@ -637,6 +639,11 @@ int ovl_group_destroy(ovl_group *g) {
 }
 
 int ovl_group_slabs(const ovl_group *g) { return g ? g->n : 0; }
+int ovl_group_set_split_launch(ovl_group *g, int on) {
+    if (!g) return OVL_EINVAL;
+    g->split_launch = on != 0;
+    return OVL_OK;
+}
 const char *ovl_group_last_error(const ovl_group *g) { return g ? g->err : "null group"; }
 long long ovl_group_launch_count(const ovl_group *g) {
     long long t = 0;

@@ -23,6 +23,10 @@ struct ovl_group {
     };
     std::vector<Wire> w;
     unsigned long long round = 0;  // launch rounds so far: round k waits on the neighbours' events of round k-1
+    // split every stencil round into a boundary launch (the two edge time slices: all halo reads and pushes), after which the
+    // round's event is recorded, and an interior launch: the neighbours' next round then overlaps this slab's interior, which
+    // hides the cross-GPU event latency.  Default: on when the slabs sit on different devices.
+    bool split_launch = false;
     int nev = 0, wcap = 0;
     unsigned defl_par = 0, red_par = 0;
     char err[256] = {0};
@@ -100,7 +104,7 @@ template <typename T> SlabArgs<T> slab_args(ovl_group *g, int r, int in_slot, in
     return a;
 }
 
-// one fused stencil launch on every slab = one round
+// one fused stencil launch (or a boundary + an interior launch) on every slab = one round
 template <typename T, int RECON, int FLAGS>
 int slab_step_t(ovl_group *g, const WilsonArgs *args, int in_slot, int out_slot) {
     constexpr int TH = WilsonCfg<T>::THREADS;
@@ -110,12 +114,25 @@ int slab_step_t(ovl_group *g, const WilsonArgs *args, int in_slot, int out_slot)
         OVL_TRY(round_begin(g, r));
         const WilsonArgs &a = args[r];
         StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)0, (T)0, a.flip};
-        k_wilson_slab<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<(c->g.V + TH - 1) / TH, TH, 0, c->st>>>(
-            c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, sp,
-            slab_args<T>(g, r, in_slot, out_slot));
-        ++c->launches;
+        const SlabArgs<T> sl = slab_args<T>(g, r, in_slot, out_slot);
+        const int ntile = (c->g.V + TH - 1) / TH, tps = c->g.sxyz / TH;  // tiles per time slice (when they align)
+        auto launch = [&](int grid, TileRange tr) {
+            k_wilson_slab<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
+                c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, sp, sl, tr);
+            ++c->launches;
+        };
+        const bool split = g->split_launch && c->g.sxyz % TH == 0 && c->g.L[3] >= 3;
+        if (split) {
+            launch(2 * tps, TileRange{0, tps, ntile - tps});         // time slices 0 and Lt-1: halo reads + pushes
+            GRP_CUDA(g, cudaGetLastError());
+            OVL_TRY(round_end(g, r));                                 // the neighbours may start their next round now
+            launch(ntile - 2 * tps, TileRange{tps, ntile, 0});        // interior
+        } else {
+            launch(ntile, TileRange{0, ntile, 0});
+            GRP_CUDA(g, cudaGetLastError());
+            OVL_TRY(round_end(g, r));
+        }
         GRP_CUDA(g, cudaGetLastError());
-        OVL_TRY(round_end(g, r));
     }
     ++g->round;
     return OVL_OK;

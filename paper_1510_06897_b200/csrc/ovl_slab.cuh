@@ -28,6 +28,14 @@ template <typename T> struct SlabArgs {
     T s_lo, s_hi;              // boundary phase of the hop across the lower / upper slab edge (-1 on the global boundary)
 };
 
+// Which tiles a launch covers: the whole slab (n1 = all tiles), or -- when the launch is split so that the neighbours can go
+// on as soon as the halo traffic is done -- the tiles of the two boundary time slices (first n1 tiles from off1, the rest
+// from off2) or the interior (one range).  Position p of the launch -> tile.
+struct TileRange {
+    int off1, n1, off2;
+    __host__ __device__ int tile(int p) const { return p < n1 ? off1 + p : off2 + (p - n1); }
+};
+
 // one hop with explicit plane strides (halo buffers and the ghost link slice are time-slice sized)
 template <typename T, int RECON, int MU, int FWD>
 __device__ __forceinline__ void hop_dir_strided(cx<T> (&hop)[12], const cx<T> *__restrict__ in, size_t in_stride, int sn,
@@ -43,9 +51,9 @@ __device__ __forceinline__ void hop_dir_strided(cx<T> (&hop)[12], const cx<T> *_
 template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_wilson_slab(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *prev,
-              const cx<T> *__restrict__ psi, cx<T> *out, const StepParams<T> sp, const SlabArgs<T> sl) {
+              const cx<T> *__restrict__ psi, cx<T> *out, const StepParams<T> sp, const SlabArgs<T> sl, const TileRange tr) {
     constexpr int NROW = RECON == 18 ? 3 : 2;
-    const int tile = sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int tile = tr.tile((int)(sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x));
     const int s = tile * THREADS + threadIdx.x;
     if (s >= g.V) return;
     const int x = s % g.L[0];

@@ -82,6 +82,14 @@ def test_host_side_argument_checks_without_gpu(lib_path):
     assert lib.ovl_create_ws(ctypes.byref(ctx), dims, ctypes.c_void_p(16), B.OVL_F64, B.OVL_RECON18, 0, 1, 0, None, 0, None) == B.OVL_EINVAL
     assert lib.ovl_create(ctypes.byref(ctx), bad, ctypes.c_void_p(16), B.OVL_F64, B.OVL_RECON18, None) == B.OVL_EINVAL
     assert lib.ovl_create(ctypes.byref(ctx), dims, None, B.OVL_F64, B.OVL_RECON18, None) == B.OVL_EINVAL
+    # the t-split group: slab arithmetic is refused before any CUDA call
+    grp = ctypes.c_void_p()
+    streams = (ctypes.c_void_p * 16)()
+    for nslabs in (0, 17, 3, 64):  # out of range; Lt = 64 not divisible by 3; Lt / nslabs < 2
+        assert lib.ovl_group_create(ctypes.byref(grp), dims, nslabs, ctypes.c_void_p(16), B.OVL_F64, B.OVL_RECON18, streams, None) == B.OVL_EINVAL
+    assert lib.ovl_group_create(ctypes.byref(grp), dims, 2, None, B.OVL_F64, B.OVL_RECON18, streams, None) == B.OVL_EINVAL
+    assert lib.ovl_group_destroy(None) == B.OVL_EINVAL and lib.ovl_group_slabs(None) == 0
+    assert lib.ovl_group_last_error(None) == b"null group"
     assert lib.ovl_destroy(None) == B.OVL_EINVAL
     assert lib.ovl_last_error(None) == b"null context"
 

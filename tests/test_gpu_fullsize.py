@@ -173,4 +173,6 @@ def test_split_lattice_full_size_bit_identical(torch, api, rough, nslabs):
             o.set_chebyshev(alpha)
         assert torch.equal(sp.dw(p), ref.dw(p))
         assert torch.equal(sp.sign(p), ref.sign(p))
+        sp.set_split_launch(True)    # boundary + interior launch per round (the multi-GPU default)
+        assert torch.equal(sp.sign(p), ref.sign(p))
         assert torch.equal(sp.overlap(p, 0.01, dagger=True), ref.overlap(p, 0.01, dagger=True))

@@ -35,10 +35,14 @@ def host(t):
     return t.detach().cpu().numpy().astype(np.complex128)
 
 
+@pytest.mark.parametrize("split_launch", [False, True])
 @pytest.mark.parametrize("nslabs", [1, 2, 4])
 @pytest.mark.parametrize("prec,recon", [("f64", 18), ("f64", 12), ("f32", 18)])
-def test_split_stencil_and_polynomial_bit_identical(torch, api, orc, nslabs, prec, recon):
-    dims = (4, 6, 4, 8)
+def test_split_stencil_and_polynomial_bit_identical(torch, api, orc, nslabs, prec, recon, split_launch):
+    """split_launch: every stencil round as a boundary launch + an interior launch with the round's event in between (the
+    multi-GPU default); 8 x 8 x 4 x 16 has 256-site time slices, i.e. whole 128-site tiles, so the split really happens
+    (for 4 slabs of 4 time slices: 4 boundary + 4 interior tiles per slab)."""
+    dims = (8, 8, 4, 16)
     U = inputs.config_links(dims, 0.4, 31, stout_steps=1)
     psi = inputs.gaussian_spinor(dims, 32)
     alpha = inputs.chebyshev_sign_coeffs(31, 0.09)
@@ -48,6 +52,7 @@ def test_split_stencil_and_polynomial_bit_identical(torch, api, orc, nslabs, pre
         p = dev(torch, psi, ref.cdtype)
         for o in (ref, sp):
             o.set_chebyshev(alpha)
+        sp.set_split_launch(split_launch)
         assert torch.equal(sp.dw(p), ref.dw(p))
         assert torch.equal(sp.khat(p), ref.khat(p))
         s_split, s_ref = sp.sign(p), ref.sign(p)
@@ -62,9 +67,10 @@ def test_split_stencil_and_polynomial_bit_identical(torch, api, orc, nslabs, pre
     assert rel_err(host(s_split), orc.sign(dims, U, alpha, psi)) < (1e-10 if prec == "f64" else 1e-5)
 
 
+@pytest.mark.parametrize("split_launch", [False, True])
 @pytest.mark.parametrize("nslabs", [2, 4])
-def test_split_deflated_overlap_and_cg(torch, api, orc, nslabs):
-    dims = (4, 4, 4, 16)
+def test_split_deflated_overlap_and_cg(torch, api, orc, nslabs, split_launch):
+    dims = (8, 4, 4, 16)
     U = inputs.config_links(dims, 0.3, 41, stout_steps=2)
     psi = inputs.gaussian_spinor(dims, 42)
     phi = inputs.orthonormal_vectors(dims, 5, 43)
@@ -76,6 +82,7 @@ def test_split_deflated_overlap_and_cg(torch, api, orc, nslabs):
         for o in (ref, sp):
             o.set_chebyshev(alpha)
             o.set_deflation(phid, lam)
+        sp.set_split_launch(split_launch)
         p = dev(torch, psi)
         y, yr = host(sp.overlap(p, mu)), host(ref.overlap(p, mu))
         yd = host(sp.overlap(p, mu, dagger=True))
