@@ -243,6 +243,26 @@ int ovl_group_khat(ovl_group *g, const void *psi, void *out);
 int ovl_group_sign(ovl_group *g, const void *psi, void *out);
 int ovl_group_overlap(ovl_group *g, double mu, int dagger, const void *psi, void *out);
 int ovl_group_cg(ovl_group *g, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out, double *true_relres_out);
+/* ONE PROCESS PER GPU (the torchrun model): each process creates the group object of ITS slab, the processes swap the
+ * export blobs (OVL_SLAB_BLOB_BYTES each; e.g. torch.distributed.all_gather) and connect.  After that the ovl_group_* calls
+ * above work unchanged, with LOCAL arguments: this rank's contiguous t-range of every canonical field / eigenvector, and
+ * every rank must make the same calls in the same order (they are collective).  The wiring is the in-process one moved
+ * behind CUDA IPC: the neighbours' halo buffers and every rank's reduction scratch are opened with cudaIpcOpenMemHandle
+ * (the fused kernels then store into / read from them directly over NVLink), the round events are interprocess events,
+ * and because a wait on an IPC event only covers records ISSUED before it, every process publishes the number of rounds it
+ * has issued in a small POSIX shared-memory segment (`shm_name`, the same string on every rank, unique per group) which
+ * the neighbours' host threads poll before they enqueue their wait.  No kernel spins; NCCL is not on the data path.
+ *   ovl_slab_create   links_local_c128 [H|D]: this rank's [V/nranks][4][3][3] complex128 links; cuda_stream: a real stream.
+ *   ovl_slab_export   fills `blob` (OVL_SLAB_BLOB_BYTES) with this rank's IPC handles.
+ *   ovl_slab_connect  `blobs`: nranks blobs in rank order; opens the other ranks' memory and events and sends this rank's
+ *                     last U_t time slice to its upper neighbour.  The caller must run a barrier across the processes
+ *                     after ovl_slab_connect and before the first collective call, and before ovl_group_destroy.
+ * Single node (CUDA IPC + POSIX shm).  Tested as two processes sharing one GPU; unmeasured across GPUs. */
+#define OVL_SLAB_BLOB_BYTES 256
+int ovl_slab_create(ovl_group **out, const int dims[4], int rank, int nranks, const void *links_local_c128, int prec, int recon,
+                    void *cuda_stream, const char *shm_name);
+int ovl_slab_export(ovl_group *g, void *blob);
+int ovl_slab_connect(ovl_group *g, const void *blobs);
 const char *ovl_group_last_error(const ovl_group *g);
 long long ovl_group_launch_count(const ovl_group *g);
 

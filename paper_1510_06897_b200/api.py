@@ -268,3 +268,42 @@ class SplitOverlap:
 
     def launch_count(self):
         return B.ovl_group_launch_count(self.grp)
+
+
+class DistributedSplitOverlap(SplitOverlap):
+    """One process per GPU (torchrun): this rank's slab of a lattice split along t over `dist.get_world_size()` ranks, wired
+    to its neighbours through CUDA IPC (include/ovl.h, ovl_slab_*).  `dist` is an initialised torch.distributed (any
+    backend: it only carries the handle exchange and the barriers).  Every method is collective; arguments and results are
+    THIS RANK'S contiguous t-range of the canonical arrays (links (V/N,4,3,3), spinors (V/N,4,3), eigenvectors (nev,V/N,4,3))."""
+
+    _counter = 0
+
+    def __init__(self, dims, links_local, dist, prec="f64", recon=18, m_w=1.5, lambda_max=6.5):
+        import os
+        torch = _torch()
+        self.dist = dist
+        self.rank, self.nslabs = dist.get_rank(), dist.get_world_size()
+        self.dims = tuple(int(d) for d in dims)
+        self.V = int(np.prod(self.dims)) // self.nslabs
+        self.prec = B.OVL_F64 if prec in ("f64", B.OVL_F64) else B.OVL_F32
+        self.devices = None
+        self.streams = [torch.cuda.Stream()]
+        name = [f"/ovl_{os.getpid()}_{DistributedSplitOverlap._counter}"]
+        DistributedSplitOverlap._counter += 1
+        dist.broadcast_object_list(name, src=0)
+        torch.cuda.synchronize()
+        self.grp = B.ovl_slab_create(self.dims, self.rank, self.nslabs, links_local, self.prec, int(recon),
+                                     self.streams[0].cuda_stream, name[0])
+        blobs = [None] * self.nslabs
+        dist.all_gather_object(blobs, B.ovl_slab_export(self.grp))
+        B.ovl_slab_connect(self.grp, b"".join(blobs))
+        dist.barrier()   # every rank's ghost links have landed before the first collective call
+        B.ovl_group_set_kernel(self.grp, m_w, lambda_max)
+        self.cdtype = torch.complex128 if self.prec == B.OVL_F64 else torch.complex64
+
+    def close(self):
+        if getattr(self, "grp", None) is not None:
+            _torch().cuda.synchronize()
+            self.dist.barrier()  # nobody unmaps memory a neighbour may still be writing
+            B.ovl_group_destroy(self.grp)
+            self.grp = None

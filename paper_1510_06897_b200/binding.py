@@ -61,6 +61,9 @@ SIGNATURES = {
     "ovl_group_sign": (_I, [_P, _P, _P]),
     "ovl_group_overlap": (_I, [_P, _D, _I, _P, _P]),
     "ovl_group_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_slab_create": (_I, [C.POINTER(_P), C.POINTER(_I), _I, _I, _P, _I, _I, _P, C.c_char_p]),
+    "ovl_slab_export": (_I, [_P, _P]),
+    "ovl_slab_connect": (_I, [_P, _P]),
     "ovl_group_last_error": (C.c_char_p, [_P]),
     "ovl_group_launch_count": (C.c_longlong, [_P]),
     "ovl_field_bytes": (C.c_size_t, [_P]),
@@ -327,6 +330,30 @@ def ovl_group_create(dims, nslabs, links, prec=OVL_F64, recon=OVL_RECON18, strea
     if rc != OVL_OK:
         raise OvlError(rc, "ovl_group_create failed")
     return g
+
+
+OVL_SLAB_BLOB_BYTES = 256
+
+
+def ovl_slab_create(dims, rank, nranks, links_local, prec=OVL_F64, recon=OVL_RECON18, stream=0, shm_name="/ovl_group"):
+    """This process's slab of a lattice split along t over `nranks` processes (one per GPU)."""
+    g = _P()
+    rc = load_library().ovl_slab_create(C.byref(g), (_I * 4)(*map(int, dims)), int(rank), int(nranks), _ptr(links_local), prec, recon,
+                                        _P(int(stream)), shm_name.encode())
+    if rc != OVL_OK:
+        raise OvlError(rc, "ovl_slab_create failed")
+    return g
+
+
+def ovl_slab_export(g) -> bytes:
+    buf = C.create_string_buffer(OVL_SLAB_BLOB_BYTES)
+    _gcheck(g, load_library().ovl_slab_export(g, buf))
+    return buf.raw
+
+
+def ovl_slab_connect(g, blobs: bytes):
+    buf = C.create_string_buffer(blobs, len(blobs))
+    return _gcheck(g, load_library().ovl_slab_connect(g, buf))
 
 
 def ovl_group_destroy(g):

@@ -4,6 +4,11 @@
 #include "ovl_eigsolve.cuh"
 #include "ovl_group.cuh"
 
+#include <fcntl.h>
+#include <sys/mman.h>
+#include <sys/stat.h>
+#include <unistd.h>
+
 using namespace ovl;
 
 #define DISPATCH(c, fn, ...) ((c)->prec == OVL_F64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
@@ -549,12 +554,61 @@ long long ovl_launch_count(const ovl_ctx *c) { return c ? c->launches : 0; }
 
 // ---------------------------------------------------------------------------------------------- t-split lattice (ovl_group)
 
+}  // extern "C"
+
+namespace {
+// one slab context + its wire block (one device allocation: halos, ghost U_t slice, reduction scratch) + its two events
+int group_add_slab(ovl_group *g, int r, const int ldims[4], const void *links_local, void *stream, bool ipc) {
+    ovl_ctx *c = nullptr;
+    const int rc = create_impl(&c, ldims, links_local, g->prec, g->recon, stream, nullptr, 0, 0, 1, 0);
+    if (rc != OVL_OK) return gfail(g, rc, "slab %d: context creation failed", r);
+    g->s[r] = c;
+    c->use_graphs = false;  // the launch sequence of a slab is interleaved with event waits on its neighbours
+    const WireLayout L = wire_layout((size_t)c->g.sxyz, c->nrow(), c->tsize());
+    void *base = nullptr;
+    GRP_CUDA(g, cudaMalloc(&base, L.total));  // its own allocation: exported as ONE IPC handle when the slabs are processes
+    c->owned.push_back(base);
+    wire_point(g->w[r], L, base);
+    for (int b = 0; b < 2; ++b)
+        GRP_CUDA(g, cudaEventCreateWithFlags(&g->w[r].ev[b], cudaEventDisableTiming | (ipc ? cudaEventInterprocess : 0)));
+    return OVL_OK;
+}
+// U_t of slab lo's last time slice -> the ghost slice of slab `to` (a peer or IPC pointer), on lo's stream
+int group_send_ghost_links(ovl_group *g, int lo, int to) {
+    ovl_ctx *cl = g->s[lo];
+    DevGuard dg(g->dev[lo]);
+    const int npl = cl->nrow() * 3;
+    const size_t ne = (size_t)npl * cl->g.sxyz;
+    if (g->prec == OVL_F64)
+        k_pack_ut_last<double><<<(unsigned)((ne + 255) / 256), 256, 0, cl->st>>>(
+            cl->g.V, cl->g.sxyz, npl, (const double2 *)cl->U + (size_t)3 * npl * cl->g.V, (double2 *)g->w[to].u_lo);
+    else
+        k_pack_ut_last<float><<<(unsigned)((ne + 255) / 256), 256, 0, cl->st>>>(
+            cl->g.V, cl->g.sxyz, npl, (const float2 *)cl->U + (size_t)3 * npl * cl->g.V, (float2 *)g->w[to].u_lo);
+    GRP_CUDA(g, cudaGetLastError());
+    GRP_CUDA(g, cudaStreamSynchronize(cl->st));
+    return OVL_OK;
+}
+int group_check(const int dims[4], int nslabs, int prec, int recon) {
+    if (check_cfg(dims, prec, recon) != OVL_OK) return OVL_EINVAL;
+    if (nslabs < 1 || nslabs > MAX_SLABS || dims[3] % nslabs != 0 || dims[3] / nslabs < 2) return OVL_EINVAL;
+    return OVL_OK;
+}
+struct SlabBlob {  // what ovl_slab_export hands to the other processes (fits OVL_SLAB_BLOB_BYTES)
+    int magic, rank;
+    cudaIpcMemHandle_t mem;
+    cudaIpcEventHandle_t ev[2];
+};
+static_assert(sizeof(SlabBlob) <= OVL_SLAB_BLOB_BYTES, "blob too large");
+}  // namespace
+
+extern "C" {
+
 int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void *links_c128, int prec, int recon,
                      void *const *cuda_streams, const int *devices) {
     if (!out) return OVL_EINVAL;
     *out = nullptr;
-    if (!links_c128 || !cuda_streams || check_cfg(dims, prec, recon) != OVL_OK) return OVL_EINVAL;
-    if (nslabs < 1 || nslabs > MAX_SLABS || dims[3] % nslabs != 0 || dims[3] / nslabs < 2) return OVL_EINVAL;
+    if (!links_c128 || !cuda_streams || group_check(dims, nslabs, prec, recon) != OVL_OK) return OVL_EINVAL;
     ovl_group *g = new (std::nothrow) ovl_group();
     if (!g) return OVL_ENOMEM;
     g->n = nslabs; g->prec = prec; g->recon = recon;
@@ -562,9 +616,10 @@ int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void 
     const int ldims[4] = {dims[0], dims[1], dims[2], dims[3] / nslabs};
     g->Vloc = (size_t)ldims[0] * ldims[1] * ldims[2] * ldims[3];
     g->w.resize(nslabs);
+    g->s.assign(nslabs, nullptr);
     int cur = 0;
     cudaGetDevice(&cur);
-    for (int r = 0; r < nslabs; ++r) g->dev.push_back(devices ? devices[r] : cur);
+    for (int r = 0; r < nslabs; ++r) { g->dev.push_back(devices ? devices[r] : cur); g->mine.push_back(r); }
     for (int r = 1; r < nslabs; ++r)
         if (g->dev[r] != g->dev[0]) g->split_launch = true;
     auto body = [&]() -> int {
@@ -577,43 +632,13 @@ int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void 
                         return gfail(g, OVL_ECUDA, "no peer access from device %d to %d: %s", g->dev[r], g->dev[q], cudaGetErrorString(e));
                     cudaGetLastError();
                 }
-        const size_t ts = prec == OVL_F64 ? 8 : 4;
         for (int r = 0; r < nslabs; ++r) {
             DevGuard dg(g->dev[r]);
-            ovl_ctx *c = nullptr;
             const char *lk = (const char *)links_c128 + (size_t)r * g->Vloc * 36 * sizeof(double2);
-            int rc = create_impl(&c, ldims, lk, prec, recon, cuda_streams[r], nullptr, 0, 0, 1, 0);
-            if (rc != OVL_OK) return gfail(g, rc, "slab %d: context creation failed", r);
-            g->s.push_back(c);
-            c->use_graphs = false;  // the launch sequence of a slab is interleaved with event waits on its neighbours
-            const size_t face = (size_t)12 * c->g.sxyz * 2 * ts;
-            for (int sl = 0; sl < 3; ++sl)
-                for (int side = 0; side < 2; ++side) GRP_TRY(g, r, dev_alloc(c, &g->w[r].halo[sl][side], face));
-            GRP_TRY(g, r, dev_alloc(c, &g->w[r].u_lo, (size_t)c->nrow() * 3 * c->g.sxyz * 2 * ts));
-            for (int b = 0; b < 2; ++b) {
-                GRP_TRY(g, r, dev_alloc(c, (void **)&g->w[r].red_loc[b], sizeof(double) * 8));
-                GRP_CUDA(g, cudaEventCreateWithFlags(&g->w[r].ev[b], cudaEventDisableTiming));
-            }
+            OVL_TRY(group_add_slab(g, r, ldims, lk, cuda_streams[r], false));
         }
         // the backward t hop of a slab's first time slice needs U_t of the lower neighbour's last slice: sent once, here
-        for (int r = 0; r < nslabs; ++r) {
-            const int lo = lo_of(g, r);
-            ovl_ctx *cl = g->s[lo];
-            DevGuard dg(g->dev[lo]);
-            const int npl = cl->nrow() * 3;
-            const size_t ne = (size_t)npl * cl->g.sxyz;
-            if (prec == OVL_F64)
-                k_pack_ut_last<double><<<(unsigned)((ne + 255) / 256), 256, 0, cl->st>>>(
-                    cl->g.V, cl->g.sxyz, npl, (const double2 *)cl->U + (size_t)3 * npl * cl->g.V, (double2 *)g->w[r].u_lo);
-            else
-                k_pack_ut_last<float><<<(unsigned)((ne + 255) / 256), 256, 0, cl->st>>>(
-                    cl->g.V, cl->g.sxyz, npl, (const float2 *)cl->U + (size_t)3 * npl * cl->g.V, (float2 *)g->w[r].u_lo);
-            GRP_CUDA(g, cudaGetLastError());
-        }
-        for (int r = 0; r < nslabs; ++r) {
-            DevGuard dg(g->dev[r]);
-            GRP_CUDA(g, cudaStreamSynchronize(g->s[r]->st));
-        }
+        for (int r = 0; r < nslabs; ++r) OVL_TRY(group_send_ghost_links(g, lo_of(g, r), r));
         return OVL_OK;
     };
     const int rc = body();
@@ -622,18 +647,104 @@ int ovl_group_create(ovl_group **out, const int dims[4], int nslabs, const void 
     return OVL_OK;
 }
 
+/* ---- one process per GPU: the same slabs, wired through CUDA IPC ---- */
+int ovl_slab_create(ovl_group **out, const int dims[4], int rank, int nranks, const void *links_local_c128, int prec, int recon,
+                    void *cuda_stream, const char *shm_name) {
+    if (!out) return OVL_EINVAL;
+    *out = nullptr;
+    if (!links_local_c128 || !shm_name || group_check(dims, nranks, prec, recon) != OVL_OK || rank < 0 || rank >= nranks) return OVL_EINVAL;
+    if (strlen(shm_name) == 0 || strlen(shm_name) >= sizeof(((ovl_group *)0)->shm_name)) return OVL_EINVAL;
+    ovl_group *g = new (std::nothrow) ovl_group();
+    if (!g) return OVL_ENOMEM;
+    g->n = nranks; g->prec = prec; g->recon = recon; g->distributed = true; g->rank = rank;
+    g->split_launch = nranks > 1;
+    for (int i = 0; i < 4; ++i) g->gdims[i] = dims[i];
+    const int ldims[4] = {dims[0], dims[1], dims[2], dims[3] / nranks};
+    g->Vloc = (size_t)ldims[0] * ldims[1] * ldims[2] * ldims[3];
+    g->w.resize(nranks);
+    g->s.assign(nranks, nullptr);
+    int cur = 0;
+    cudaGetDevice(&cur);
+    g->dev.assign(nranks, cur);
+    g->mine.push_back(rank);
+    strcpy(g->shm_name, shm_name);
+    auto body = [&]() -> int {
+        // "rounds issued" counters shared by the processes of the group (a record must have been issued before a wait on it)
+        const size_t bytes = sizeof(unsigned long long) * MAX_SLABS;
+        const int fd = shm_open(shm_name, O_CREAT | O_RDWR, 0600);
+        if (fd < 0) return gfail(g, OVL_ECUDA, "shm_open(%s) failed", shm_name);
+        if (ftruncate(fd, (off_t)bytes) != 0) { close(fd); return gfail(g, OVL_ECUDA, "ftruncate on %s failed", shm_name); }
+        void *m = mmap(nullptr, bytes, PROT_READ | PROT_WRITE, MAP_SHARED, fd, 0);
+        close(fd);
+        if (m == MAP_FAILED) return gfail(g, OVL_ECUDA, "mmap of %s failed", shm_name);
+        g->issued = (volatile unsigned long long *)m;
+        __atomic_store_n(&g->issued[rank], 0ull, __ATOMIC_RELEASE);
+        return group_add_slab(g, rank, ldims, links_local_c128, cuda_stream, true);
+    };
+    const int rc = body();
+    if (rc != OVL_OK) { ovl_group_destroy(g); return rc; }
+    *out = g;
+    return OVL_OK;
+}
+
+int ovl_slab_export(ovl_group *g, void *blob) {
+    if (!g || !blob || !g->distributed) return OVL_EINVAL;
+    SlabBlob b;
+    memset(&b, 0, sizeof b);
+    b.magic = 0x0516a5b; b.rank = g->rank;
+    DevGuard dg(g->dev[g->rank]);
+    GRP_CUDA(g, cudaIpcGetMemHandle(&b.mem, g->w[g->rank].base));
+    for (int i = 0; i < 2; ++i) GRP_CUDA(g, cudaIpcGetEventHandle(&b.ev[i], g->w[g->rank].ev[i]));
+    memset(blob, 0, OVL_SLAB_BLOB_BYTES);
+    memcpy(blob, &b, sizeof b);
+    return OVL_OK;
+}
+
+int ovl_slab_connect(ovl_group *g, const void *blobs) {
+    if (!g || !blobs || !g->distributed) return OVL_EINVAL;
+    ovl_ctx *c = g->s[g->rank];
+    DevGuard dg(g->dev[g->rank]);
+    const WireLayout L = wire_layout((size_t)c->g.sxyz, c->nrow(), c->tsize());
+    for (int q = 0; q < g->n; ++q) {
+        if (q == g->rank) continue;
+        SlabBlob b;
+        memcpy(&b, (const char *)blobs + (size_t)q * OVL_SLAB_BLOB_BYTES, sizeof b);
+        if (b.magic != 0x0516a5b || b.rank != q) return gfail(g, OVL_EINVAL, "blob %d is not the export of slab %d", q, q);
+        void *base = nullptr;
+        GRP_CUDA(g, cudaIpcOpenMemHandle(&base, b.mem, cudaIpcMemLazyEnablePeerAccess));
+        wire_point(g->w[q], L, base);
+        g->w[q].remote = true;
+        for (int i = 0; i < 2; ++i) GRP_CUDA(g, cudaIpcOpenEventHandle(&g->w[q].ev[i], b.ev[i]));
+    }
+    // my last U_t slice is the upper neighbour's ghost slice (the caller runs a barrier across the processes after this call)
+    return group_send_ghost_links(g, g->rank, hi_of(g, g->rank));
+}
+
 int ovl_group_destroy(ovl_group *g) {
     if (!g) return OVL_EINVAL;
-    for (size_t r = 0; r < g->s.size(); ++r) {
-        DevGuard dg(g->dev[r]);
-        cudaStreamSynchronize(g->s[r]->st);
+    for (int r : g->mine)
+        if (g->s[r]) {
+            DevGuard dg(g->dev[r]);
+            cudaStreamSynchronize(g->s[r]->st);
+        }
+    for (size_t q = 0; q < g->w.size(); ++q) {
+        if (g->w[q].remote) {
+            if (g->w[q].base) cudaIpcCloseMemHandle(g->w[q].base);
+            for (int b = 0; b < 2; ++b)
+                if (g->w[q].ev[b]) cudaEventDestroy(g->w[q].ev[b]);
+        }
     }
-    for (size_t r = 0; r < g->s.size(); ++r) {
+    for (int r : g->mine) {
         DevGuard dg(g->dev[r]);
         for (int b = 0; b < 2; ++b)
             if (g->w[r].ev[b]) cudaEventDestroy(g->w[r].ev[b]);
-        ovl_destroy(g->s[r]);
+        if (g->s[r]) ovl_destroy(g->s[r]);
     }
+    if (g->issued) {
+        munmap((void *)g->issued, sizeof(unsigned long long) * MAX_SLABS);
+        if (g->rank == 0) shm_unlink(g->shm_name);
+    }
+    cudaGetLastError();
     delete g;
     return OVL_OK;
 }
@@ -647,34 +758,31 @@ int ovl_group_set_split_launch(ovl_group *g, int on) {
 const char *ovl_group_last_error(const ovl_group *g) { return g ? g->err : "null group"; }
 long long ovl_group_launch_count(const ovl_group *g) {
     long long t = 0;
-    if (g) for (ovl_ctx *c : g->s) t += c->launches;
+    if (g) for (int r : g->mine) t += g->s[r]->launches;
     return t;
 }
 
 int ovl_group_set_kernel(ovl_group *g, double m_w, double lambda_max) {
     if (!g) return OVL_EINVAL;
-    for (int r = 0; r < g->n; ++r) GRP_TRY(g, r, ovl_set_kernel(g->s[r], m_w, lambda_max));
+    for (int r : g->mine) GRP_TRY(g, r, ovl_set_kernel(g->s[r], m_w, lambda_max));
     return OVL_OK;
 }
 int ovl_group_set_chebyshev(ovl_group *g, int N, const double *alpha) {
     if (!g) return OVL_EINVAL;
-    for (int r = 0; r < g->n; ++r) GRP_TRY(g, r, ovl_set_chebyshev(g->s[r], N, alpha));
+    for (int r : g->mine) GRP_TRY(g, r, ovl_set_chebyshev(g->s[r], N, alpha));
     return OVL_OK;
 }
 int ovl_group_set_deflation(ovl_group *g, int nev, const void *phi, const double *lambda) {
     if (!g) return OVL_EINVAL;
-    const size_t vstride = (size_t)g->n * g->Vloc * 12 * sizeof(double2);  // one GLOBAL eigenvector
-    for (int r = 0; r < g->n; ++r) {
+    if (nev > WIRE_MAX_NEV) return gfail(g, OVL_EINVAL, "at most %d deflation vectors on a split lattice", WIRE_MAX_NEV);
+    // phi holds, per eigenvector, the parts of this process's slabs back to back (all slabs: the global vector)
+    const size_t vstride = g->mine.size() * g->Vloc * 12 * sizeof(double2);
+    for (size_t li = 0; li < g->mine.size(); ++li) {
+        const int r = g->mine[li];
         DevGuard dg(g->dev[r]);
-        const char *p = phi ? (const char *)phi + (size_t)r * g->Vloc * 12 * sizeof(double2) : nullptr;
+        const char *p = phi ? (const char *)phi + li * g->Vloc * 12 * sizeof(double2) : nullptr;
         GRP_TRY(g, r, set_deflation_strided(g->s[r], nev, p, lambda, vstride));
-        if (nev > g->wcap)
-            for (int b = 0; b < 2; ++b) {
-                dev_release(g->s[r], (void **)&g->w[r].w_loc[b]);
-                GRP_TRY(g, r, dev_alloc(g->s[r], (void **)&g->w[r].w_loc[b], sizeof(double2) * nev));
-            }
     }
-    if (nev > g->wcap) g->wcap = nev;
     g->nev = nev;
     return OVL_OK;
 }
@@ -686,21 +794,23 @@ namespace {
 template <typename F> int group_with_canonical(ovl_group *g, const void *psi, void *out, F body) {
     if (!g) return OVL_EINVAL;
     if (!psi || !out || psi == out) return gfail(g, OVL_EINVAL, "null or aliased spinor pointers");
-    std::vector<void *> in(g->n), o(g->n);
-    for (int r = 0; r < g->n; ++r) {
+    std::vector<void *> in(g->n, nullptr), o(g->n, nullptr);
+    for (size_t li = 0; li < g->mine.size(); ++li) {  // this process's slabs lie back to back in psi / out
+        const int r = g->mine[li];
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
-        GRP_TRY(g, r, import_any(c, (const char *)psi + (size_t)r * c->canon_bytes(), c->psi_n));
+        GRP_TRY(g, r, import_any(c, (const char *)psi + li * c->canon_bytes(), c->psi_n));
         in[r] = c->psi_n; o[r] = c->out_n;
     }
     const int rc = body(in.data(), o.data());
     if (rc != OVL_OK && rc != OVL_ENOTCONV) return rc;
-    for (int r = 0; r < g->n; ++r) {
+    for (size_t li = 0; li < g->mine.size(); ++li) {
+        const int r = g->mine[li];
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
-        GRP_TRY(g, r, export_any(c, c->out_n, (char *)out + (size_t)r * c->canon_bytes()));
+        GRP_TRY(g, r, export_any(c, c->out_n, (char *)out + li * c->canon_bytes()));
     }
-    for (int r = 0; r < g->n; ++r) {  // the group calls synchronise: their result spans several streams
+    for (int r : g->mine) {  // the group calls synchronise: their result spans several streams
         DevGuard dg(g->dev[r]);
         GRP_CUDA(g, cudaStreamSynchronize(g->s[r]->st));
     }
@@ -726,7 +836,7 @@ int ovl_group_overlap(ovl_group *g, double mu, int dagger, const void *psi, void
 int ovl_group_cg(ovl_group *g, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out, double *relres_out) {
     if (!g) return OVL_EINVAL;
     if (!iters_out || !relres_out || maxiter < 0) return gfail(g, OVL_EINVAL, "bad ovl_group_cg arguments");
-    if (g->s[0]->alpha.empty()) return gfail(g, OVL_ESTATE, "ovl_group_set_chebyshev has not been called");
+    if (g->s[g->mine[0]]->alpha.empty()) return gfail(g, OVL_ESTATE, "ovl_group_set_chebyshev has not been called");
     return group_with_canonical(g, b, x, [&](void *const *i, void *const *o) { return GDISPATCH(g, group_cg, g, mu, i, o, tol, maxiter, iters_out, relres_out); });
 }
 

@@ -5,14 +5,18 @@
 #include "ovl_engine.cuh"
 #include "ovl_slab.cuh"
 
+#include <chrono>
+
 struct ovl_group {
-    int n = 0;
+    int n = 0;                 // slabs of the lattice
     int gdims[4] = {0, 0, 0, 0};
     int prec = OVL_F64, recon = OVL_RECON18;
     size_t Vloc = 0;
-    std::vector<ovl_ctx *> s;  // slab contexts: local lattice Lx x Ly x Lz x (Lt / n)
-    std::vector<int> dev;      // device ordinal per slab
-    struct Wire {
+    std::vector<ovl_ctx *> s;  // slab contexts (local lattice Lx x Ly x Lz x (Lt / n)); null for slabs of other processes
+    std::vector<int> mine;     // the slabs this process runs: all of them (in-process group) or one (one process per GPU)
+    std::vector<int> dev;      // device ordinal per local slab (index = slab)
+    struct Wire {              // what a slab exposes to the others: all of it lives in ONE device allocation (one IPC handle)
+        void *base = nullptr;
         void *halo[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};  // [slot][lo / hi], one time slice each
         void *u_lo = nullptr;                                                            // ghost U_t slice
         // this slab's share of the deflation coefficients (2 nev doubles) / of a CG scalar; two buffers used alternately, so a
@@ -20,6 +24,7 @@ struct ovl_group {
         double *w_loc[2] = {nullptr, nullptr};
         double *red_loc[2] = {nullptr, nullptr};
         cudaEvent_t ev[2] = {nullptr, nullptr};
+        bool remote = false;   // opened through CUDA IPC (another process)
     };
     std::vector<Wire> w;
     unsigned long long round = 0;  // launch rounds so far: round k waits on the neighbours' events of round k-1
@@ -27,8 +32,14 @@ struct ovl_group {
     // round's event is recorded, and an interior launch: the neighbours' next round then overlaps this slab's interior, which
     // hides the cross-GPU event latency.  Default: on when the slabs sit on different devices.
     bool split_launch = false;
-    int nev = 0, wcap = 0;
+    int nev = 0;
     unsigned defl_par = 0, red_par = 0;
+    // one process per GPU: a record must have been ISSUED by the neighbour's host thread before this process may wait on
+    // the (IPC) event, so every process publishes "rounds issued so far" in a small POSIX shared-memory segment
+    bool distributed = false;
+    int rank = 0;
+    volatile unsigned long long *issued = nullptr;  // [n], shared between the processes of the group
+    char shm_name[96] = {0};
     char err[256] = {0};
 };
 
@@ -66,6 +77,41 @@ inline int gfail(ovl_group *g, int code, const char *fmt, ...) {
         if (rc_ != OVL_OK) return ovl::gfail((g), rc_, "slab %d: %s", (r), (g)->s[(r)]->err);    \
     } while (0)
 
+constexpr int WIRE_MAX_NEV = 512;  // capacity of the deflation-coefficient scratch (fixed so the layout never changes)
+struct WireLayout { size_t halo[3][2], u_lo, w_loc[2], red_loc[2], total; };
+inline WireLayout wire_layout(size_t sxyz, int nrow, size_t ts) {
+    WireLayout L;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += ws_round(bytes); return o; };
+    for (int sl = 0; sl < 3; ++sl)
+        for (int side = 0; side < 2; ++side) L.halo[sl][side] = take(12 * sxyz * 2 * ts);
+    L.u_lo = take((size_t)nrow * 3 * sxyz * 2 * ts);
+    for (int b = 0; b < 2; ++b) L.w_loc[b] = take(sizeof(double2) * WIRE_MAX_NEV);
+    for (int b = 0; b < 2; ++b) L.red_loc[b] = take(sizeof(double) * 8);
+    L.total = off;
+    return L;
+}
+inline void wire_point(ovl_group::Wire &w, const WireLayout &L, void *base) {
+    char *p = (char *)base;
+    w.base = base;
+    for (int sl = 0; sl < 3; ++sl)
+        for (int side = 0; side < 2; ++side) w.halo[sl][side] = p + L.halo[sl][side];
+    w.u_lo = p + L.u_lo;
+    for (int b = 0; b < 2; ++b) { w.w_loc[b] = (double *)(p + L.w_loc[b]); w.red_loc[b] = (double *)(p + L.red_loc[b]); }
+}
+
+// one process per GPU: block (on the host) until slab q's process has issued the record of round `need - 1`
+inline int wait_issued(ovl_group *g, int q, unsigned long long need) {
+    if (!g->distributed || g->s[q] != nullptr) return OVL_OK;
+    const auto t0 = std::chrono::steady_clock::now();
+    unsigned spins = 0;
+    while (__atomic_load_n(&g->issued[q], __ATOMIC_ACQUIRE) < need) {
+        if ((++spins & 0xfff) == 0 && std::chrono::steady_clock::now() - t0 > std::chrono::seconds(60))
+            return gfail(g, OVL_ECUDA, "slab %d did not issue round %llu within 60 s", q, need - 1);
+    }
+    return OVL_OK;
+}
+
 inline int lo_of(const ovl_group *g, int r) { return (r + g->n - 1) % g->n; }
 inline int hi_of(const ovl_group *g, int r) { return (r + 1) % g->n; }
 
@@ -74,12 +120,17 @@ inline int hi_of(const ovl_group *g, int r) { return (r + 1) % g->n; }
 inline int round_begin(ovl_group *g, int r) {
     if (g->round == 0) return OVL_OK;
     const int p = (int)((g->round - 1) & 1);
+    OVL_TRY(wait_issued(g, lo_of(g, r), g->round));
     GRP_CUDA(g, cudaStreamWaitEvent(g->s[r]->st, g->w[lo_of(g, r)].ev[p], 0));
-    if (hi_of(g, r) != lo_of(g, r)) GRP_CUDA(g, cudaStreamWaitEvent(g->s[r]->st, g->w[hi_of(g, r)].ev[p], 0));
+    if (hi_of(g, r) != lo_of(g, r)) {
+        OVL_TRY(wait_issued(g, hi_of(g, r), g->round));
+        GRP_CUDA(g, cudaStreamWaitEvent(g->s[r]->st, g->w[hi_of(g, r)].ev[p], 0));
+    }
     return OVL_OK;
 }
 inline int round_end(ovl_group *g, int r) {
     GRP_CUDA(g, cudaEventRecord(g->w[r].ev[g->round & 1], g->s[r]->st));
+    if (g->distributed) __atomic_store_n(&g->issued[r], g->round + 1, __ATOMIC_RELEASE);
     return OVL_OK;
 }
 // a round in which every slab waits for EVERY slab's previous round (reductions over slabs)
@@ -87,7 +138,10 @@ inline int round_begin_all(ovl_group *g, int r) {
     if (g->round == 0) return OVL_OK;
     const int p = (int)((g->round - 1) & 1);
     for (int q = 0; q < g->n; ++q)
-        if (q != r) GRP_CUDA(g, cudaStreamWaitEvent(g->s[r]->st, g->w[q].ev[p], 0));
+        if (q != r) {
+            OVL_TRY(wait_issued(g, q, g->round));
+            GRP_CUDA(g, cudaStreamWaitEvent(g->s[r]->st, g->w[q].ev[p], 0));
+        }
     return OVL_OK;
 }
 
@@ -108,7 +162,7 @@ template <typename T> SlabArgs<T> slab_args(ovl_group *g, int r, int in_slot, in
 template <typename T, int RECON, int FLAGS>
 int slab_step_t(ovl_group *g, const WilsonArgs *args, int in_slot, int out_slot) {
     constexpr int TH = WilsonCfg<T>::THREADS;
-    for (int r = 0; r < g->n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         OVL_TRY(round_begin(g, r));
@@ -143,7 +197,7 @@ template <typename T, int FLAGS> int slab_step(ovl_group *g, const WilsonArgs *a
 
 // push the faces of field f_r (one per slab) into the neighbours' halo slot: one round
 template <typename T> int push_faces(ovl_group *g, void *const *f, int slot) {
-    for (int r = 0; r < g->n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         OVL_TRY(round_begin(g, r));
@@ -163,7 +217,7 @@ template <typename T> int push_faces(ovl_group *g, void *const *f, int slot) {
 template <typename T> int group_stencil(ovl_group *g, int g5, void *const *in, void *const *out) {
     OVL_TRY(push_faces<T>(g, in, SLOT_SRC));
     std::vector<WilsonArgs> a(g->n);
-    for (int r = 0; r < g->n; ++r) {
+    for (int r : g->mine) {
         a[r].in = in[r]; a[r].out = out[r];
         a[r].c_diag = g5 ? (4.0 - g->s[r]->m_w) / g->s[r]->lambda_max : 4.0;
         a[r].c_hop = g5 ? -0.5 / g->s[r]->lambda_max : -0.5;
@@ -173,7 +227,7 @@ template <typename T> int group_stencil(ovl_group *g, int g5, void *const *in, v
 
 // acc_r = sum_m alpha_m T_m(K^) src_r by Clenshaw's recurrence, the launch sequence of cheb_clenshaw() on every slab
 template <typename T> int group_cheb(ovl_group *g, void *const *src) {
-    ovl_ctx *c0 = g->s[0];
+    ovl_ctx *c0 = g->s[g->mine[0]];
     const double cd = (4.0 - c0->m_w) / c0->lambda_max, ch = -0.5 / c0->lambda_max;
     const std::vector<double> &al = c0->alpha;
     const int N = c0->norders, n = g->n;
@@ -187,7 +241,7 @@ template <typename T> int group_cheb(ovl_group *g, void *const *src) {
         return which == 0 ? src[r] : which == 1 ? c->tA : which == 2 ? c->tB : c->acc;
     };
     auto step = [&](int in, int prev, int out, double scale, double a_psi) -> int {
-        for (int r = 0; r < n; ++r) {
+        for (int r : g->mine) {
             a[r] = WilsonArgs();
             a[r].in = buf(r, in); a[r].prev = prev >= 0 ? buf(r, prev) : nullptr; a[r].psi = src[r]; a[r].out = buf(r, out);
             a[r].c_diag = scale * cd; a[r].c_hop = scale * ch; a[r].a_psi = a_psi; a[r].flip = nl & 1;
@@ -213,9 +267,9 @@ template <typename T> int group_cheb(ovl_group *g, void *const *src) {
 // out_r = a in_r + b [gamma5] sign(K) src_r on the split lattice (see sign_combine_native); chir as there
 template <typename T> int group_sign_combine(ovl_group *g, double a, double b, int dagger, int g5out, void *const *in, void *const *out, int chir = 0) {
     const int n = g->n;
-    if (g->s[0]->alpha.empty()) return gfail(g, OVL_ESTATE, "ovl_group_set_chebyshev has not been called");
+    if (g->s[g->mine[0]]->alpha.empty()) return gfail(g, OVL_ESTATE, "ovl_group_set_chebyshev has not been called");
     std::vector<void *> src(n);
-    for (int r = 0; r < n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         const size_t ne = c->n(), n_upper = (size_t)6 * c->g.V;
@@ -236,12 +290,12 @@ template <typename T> int group_sign_combine(ovl_group *g, double a, double b, i
     }
     OVL_TRY(group_cheb<T>(g, src.data()));
     if (g->nev > 0) {  // w_i = sum over slabs, in slab order, on every slab (the tiny all-reduce of SURVEY §8(e))
-        for (int r = 0; r < n; ++r) { DevGuard dg(g->dev[r]); OVL_TRY(round_end(g, r)); }
+        for (int r : g->mine) { DevGuard dg(g->dev[r]); OVL_TRY(round_end(g, r)); }
         ++g->round;
         SlabPtrs parts;
         for (int q = 0; q < n; ++q) parts.p[q] = g->w[q].w_loc[g->defl_par & 1];
         ++g->defl_par;
-        for (int r = 0; r < n; ++r) {
+        for (int r : g->mine) {
             ovl_ctx *c = g->s[r];
             DevGuard dg(g->dev[r]);
             OVL_TRY(round_begin_all(g, r));
@@ -251,7 +305,7 @@ template <typename T> int group_sign_combine(ovl_group *g, double a, double b, i
         }
         ++g->round;
     }
-    for (int r = 0; r < n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         const size_t ne = c->n(), n_upper = (size_t)6 * c->g.V;
@@ -284,7 +338,7 @@ __global__ void k_cg_scalars_slabs(int nslabs, SlabPtrs locs, double *sc, int wh
 }
 inline int group_scalar(ovl_group *g, int what, double tol2) {
     const int n = g->n;
-    for (int r = 0; r < n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         k_slab_total<<<1, BLAS_THREADS, 0, c->st>>>(c->red_nblk, c->red_partial, g->w[r].red_loc[g->red_par & 1]);
@@ -295,7 +349,7 @@ inline int group_scalar(ovl_group *g, int what, double tol2) {
     SlabPtrs locs;
     for (int q = 0; q < n; ++q) locs.p[q] = g->w[q].red_loc[g->red_par & 1];
     ++g->red_par;
-    for (int r = 0; r < n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         OVL_TRY(round_begin_all(g, r));
@@ -314,7 +368,7 @@ template <typename T>
 int group_cg(ovl_group *g, double mu, void *const *b, void *const *x, double tol, int maxiter, int *iters, double *relres) {
     const int n = g->n;
     std::vector<void *> r_(n), p_(n), q_(n), Ap_(n);
-    for (int r = 0; r < n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         GRP_TRY(g, r, ensure_cg(c, 1));
@@ -327,9 +381,9 @@ int group_cg(ovl_group *g, double mu, void *const *b, void *const *x, double tol
         ++c->launches;
     }
     OVL_TRY(group_scalar(g, 0, 0.0));
-    ovl_ctx *c0 = g->s[0];
+    ovl_ctx *c0 = g->s[g->mine[0]];
     auto fetch0 = [&]() -> int {
-        DevGuard dg(g->dev[0]);
+        DevGuard dg(g->dev[g->mine[0]]);
         GRP_CUDA(g, cudaMemcpyAsync(c0->sc_host, c0->sc_dev, sizeof(double) * SC_N, cudaMemcpyDeviceToHost, c0->st));
         GRP_CUDA(g, cudaStreamSynchronize(c0->st));
         return OVL_OK;
@@ -342,14 +396,14 @@ int group_cg(ovl_group *g, double mu, void *const *b, void *const *x, double tol
     while (it < maxiter && !conv) {
         OVL_TRY(group_overlap<T>(g, mu, 0, p_.data(), q_.data()));
         OVL_TRY(group_overlap<T>(g, mu, 1, q_.data(), Ap_.data()));
-        for (int r = 0; r < n; ++r) {
+        for (int r : g->mine) {
             ovl_ctx *c = g->s[r];
             DevGuard dg(g->dev[r]);
             k_redot<T><<<dim3(c->red_nblk, 1), BLAS_THREADS, 0, c->st>>>(c->n(), (const cx<T> *)c->cg_p, (const cx<T> *)c->cg_Ap, c->red_partial);
             ++c->launches;
         }
         OVL_TRY(group_scalar(g, 1, 0.0));
-        for (int r = 0; r < n; ++r) {
+        for (int r : g->mine) {
             ovl_ctx *c = g->s[r];
             DevGuard dg(g->dev[r]);
             k_cg_update<T><<<dim3(c->red_nblk, 1), BLAS_THREADS, 0, c->st>>>(c->n(), c->sc_dev, (const cx<T> *)c->cg_p, (const cx<T> *)c->cg_Ap,
@@ -357,7 +411,7 @@ int group_cg(ovl_group *g, double mu, void *const *b, void *const *x, double tol
             ++c->launches;
         }
         OVL_TRY(group_scalar(g, 2, tol2));
-        for (int r = 0; r < n; ++r) {
+        for (int r : g->mine) {
             ovl_ctx *c = g->s[r];
             DevGuard dg(g->dev[r]);
             k_xpay<T><<<dim3(grid_for(c->n(), BLAS_THREADS), 1), BLAS_THREADS, 0, c->st>>>(c->n(), c->sc_dev, (const cx<T> *)c->cg_r, (cx<T> *)c->cg_p);
@@ -372,7 +426,7 @@ int group_cg(ovl_group *g, double mu, void *const *b, void *const *x, double tol
     *iters = it;
     OVL_TRY(group_overlap<T>(g, mu, 0, x, q_.data()));
     OVL_TRY(group_overlap<T>(g, mu, 1, q_.data(), Ap_.data()));
-    for (int r = 0; r < n; ++r) {
+    for (int r : g->mine) {
         ovl_ctx *c = g->s[r];
         DevGuard dg(g->dev[r]);
         k_sub<T><<<dim3(grid_for(c->n(), BLAS_THREADS), 1), BLAS_THREADS, 0, c->st>>>(c->n(), (const cx<T> *)b[r], (const cx<T> *)c->cg_Ap, (cx<T> *)c->cg_q);
