@@ -574,52 +574,74 @@ def run_profile_target(args, w):
 
 
 def run_tsplit(args, w):
-    """--parallelism tsplit: ONE lattice split along t over the N GPUs of the node (ovl_group_*: one slab per GPU, halo stores
-    fused into the stencil kernel as NVLink peer stores, event-ordered).  The group lives in one process, so under torchrun
-    rank 0 drives all N devices and the other ranks leave at once.  "scaling": "strong" (the lattice is fixed).  Canonical
-    fields in, canonical fields out (device resident); no deflation vectors are timed here -- the split context's timing
-    hooks cover whole applies only."""
+    """--parallelism tsplit: ONE lattice split along t over the N GPUs of the node, halo stores fused into the stencil
+    kernel as NVLink peer stores, event-ordered (include/ovl.h, ovl_group_* / ovl_slab_*).  "scaling": "strong" (the lattice
+    is fixed).  Under torchrun: one process per GPU, slabs wired through CUDA IPC (DistributedSplitOverlap), each rank
+    holds its t-range of every field; without torchrun: one process drives all N devices (SplitOverlap).  Timed: canonical
+    device-resident fields in, canonical fields out, barrier + synchronize around K applies, max over ranks."""
     import torch
 
     from paper_1510_06897_b200 import api, binding as B, build
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return
     if build.needs_build():
         build.build_library()
     B.load_library()
+    rank, local, world = replicas.world()
     n = args.gpus
-    ndev = torch.cuda.device_count()
-    devices = list(range(n)) if ndev >= n else [0] * n   # fewer GPUs than slabs: several slabs share a device (test mode)
-    torch.cuda.set_device(devices[0])
     U, psi, alpha, phi, lam = make_inputs(w)
-    Ud = torch.from_numpy(U).cuda()
-    p = torch.from_numpy(psi).cuda()
-    with api.SplitOverlap(w["dims"], Ud, n, args.prec, args.recon, devices=devices if ndev >= n else None) as sp:
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        torch.cuda.set_device(local)
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+        V = int(np.prod(w["dims"]))
+        sl = slice(rank * (V // world), (rank + 1) * (V // world))
+        sp = api.DistributedSplitOverlap(w["dims"], torch.from_numpy(np.ascontiguousarray(U[sl])).cuda(), dist, args.prec, args.recon)
+        p = torch.from_numpy(np.ascontiguousarray(psi[sl])).cuda().to(sp.cdtype)
+        phid = torch.from_numpy(np.ascontiguousarray(phi[:, sl])).cuda()
+        mode = f"tsplit x{world}: one process per GPU, CUDA IPC halos"
+    else:
+        ndev = torch.cuda.device_count()
+        devices = list(range(n)) if ndev >= n else None   # fewer GPUs than slabs: the slabs share a device (test mode)
+        torch.cuda.set_device(0)
+        sp = api.SplitOverlap(w["dims"], torch.from_numpy(U).cuda(), n, args.prec, args.recon, devices=devices)
+        p = torch.from_numpy(psi).cuda().to(sp.cdtype)
+        phid = torch.from_numpy(phi).cuda()
+        mode = f"tsplit x{n}: one process, " + (f"{n} devices" if devices else f"{n} slabs sharing {ndev} GPU(s) (test mode)")
+    try:
         sp.set_chebyshev(alpha)
-        sp.set_deflation(torch.from_numpy(phi).cuda(), lam)
+        sp.set_deflation(phid, lam)
+        del phid
         for _ in range(args.warmup):
             y = sp.overlap(p, w["mu"])
+        if dist is not None:
+            dist.barrier()
         torch.cuda.synchronize()
-        sampler = ClockSampler(devices[0]).start()
+        sampler = ClockSampler(torch.cuda.current_device()).start()
         l0 = sp.launch_count()
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            y = sp.overlap(p, w["mu"])   # synchronises every slab stream before returning
-        dt = time.perf_counter() - t0
+            y = sp.overlap(p, w["mu"])   # synchronises this process's slab streams before returning
+        torch.cuda.synchronize()
+        ms = replicas.max_over_ranks(1e3 * (time.perf_counter() - t0), dist, "cuda")
         clocks = sampler.stop()
         launches = sp.launch_count() - l0
-    val = args.steps / dt
-    line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": n, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-            "dtype": args.prec, "data": "synthetic",
-            "config": {"workload": w["desc"], "precision": args.prec, "links": f"{args.recon}-real",
-                       "parallelism": f"tsplit x{n} (one lattice, {n} slabs along t" + (")" if ndev >= n else f", all on {ndev} GPU(s): test mode)"),
-                       "timing": "host clock around calls that synchronise all slab streams (canonical device-resident fields in and out)"},
-            "clocks": clocks, "gpu_launches": launches,
-            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
-                    "note": "device-resident canonical fields; the replicas arm carries the host-buffer e2e number"}}
-    print(json.dumps(line))
+        finite = bool(torch.isfinite(torch.view_as_real(y)).all().item())
+    finally:
+        sp.close()
+    if rank == 0:
+        val = args.steps / (ms * 1e-3)
+        line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": n, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": args.prec, "data": "synthetic",
+                "config": {"workload": w["desc"], "precision": args.prec, "links": f"{args.recon}-real", "parallelism": mode,
+                           "timing": "host clock around collective calls that synchronise the slab streams, max over ranks"},
+                "clocks": clocks, "gpu_launches": launches, "extras": {"finite": finite},
+                "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                        "note": "device-resident canonical fields; the replicas arm carries the host-buffer e2e number"}}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
 
 
 def run_native(args, w):
