@@ -69,11 +69,12 @@ __device__ __forceinline__ double block_sum(double v, double *sm) {
 // The reduction tree per (r, i) -- thread-serial over the chunk, warp shuffle, warps 0..7 in order -- does not depend on
 // the group size, so a right-hand side gets bit-identical coefficients whether it is projected alone or in a batch.
 constexpr int PROJ_EPT = 4;   // elements per thread
+constexpr int PROJ_IB = 4;    // eigenvectors per pass of the loop: PROJ_IB * PROJ_EPT loads in flight per thread, one barrier
 constexpr int DEFL_RB = 4;    // right-hand sides per group
 template <typename T>
-__global__ void __launch_bounds__(BLAS_THREADS)
+__global__ void __launch_bounds__(BLAS_THREADS, 2)
 k_project(size_t n, int nev, int nrhs, const cx<T> *__restrict__ phi, const cx<T> *__restrict__ psi, double2 *__restrict__ partial) {
-    __shared__ double sm[2][BLAS_THREADS / 32][2 * DEFL_RB];
+    __shared__ double sm[2][PROJ_IB][BLAS_THREADS / 32][2 * DEFL_RB];
     const size_t base = (size_t)blockIdx.x * (BLAS_THREADS * PROJ_EPT) + threadIdx.x;
     const int r0 = blockIdx.y * DEFL_RB;
     const int nr = min(DEFL_RB, nrhs - r0);
@@ -86,36 +87,49 @@ k_project(size_t n, int nev, int nrhs, const cx<T> *__restrict__ phi, const cx<T
             const size_t e = base + (size_t)j * BLAS_THREADS;
             p[r][j] = (r < nr && e < n) ? psi[(size_t)(r0 + r) * n + e] : mk<T>(0, 0);
         }
-    for (int i = 0; i < nev; ++i) {
-        const cx<T> *ph = phi + (size_t)i * n;
-        cx<T> f[PROJ_EPT];
+    for (int i0 = 0, pass = 0; i0 < nev; i0 += PROJ_IB, ++pass) {
+        // all loads of the pass first (the eigenvector stream is the whole traffic of this kernel) ...
+        cx<T> f[PROJ_IB][PROJ_EPT];
 #pragma unroll
-        for (int j = 0; j < PROJ_EPT; ++j) {
-            const size_t e = base + (size_t)j * BLAS_THREADS;
-            f[j] = e < n ? ldg(ph + e) : mk<T>(0, 0);
+        for (int q = 0; q < PROJ_IB; ++q) {
+            const cx<T> *ph = phi + (size_t)min(i0 + q, nev - 1) * n;
+#pragma unroll
+            for (int j = 0; j < PROJ_EPT; ++j) {
+                const size_t e = base + (size_t)j * BLAS_THREADS;
+                f[q][j] = e < n ? ldg(ph + e) : mk<T>(0, 0);
+            }
         }
-        double (*buf)[2 * DEFL_RB] = sm[i & 1];
+        // ... then, per eigenvector, exactly the tree of the one-vector-per-pass version: thread-serial over j, warp
+        // shuffle, warps in order
 #pragma unroll
-        for (int r = 0; r < DEFL_RB; ++r) {
-            if (r < nr) {
-                double re = 0, im = 0;
+        for (int q = 0; q < PROJ_IB; ++q) {
+            double (*buf)[2 * DEFL_RB] = sm[pass & 1][q];
 #pragma unroll
-                for (int j = 0; j < PROJ_EPT; ++j) {
-                    if (base + (size_t)j * BLAS_THREADS < n) {
-                        re += (double)f[j].x * (double)p[r][j].x + (double)f[j].y * (double)p[r][j].y;
-                        im += (double)f[j].x * (double)p[r][j].y - (double)f[j].y * (double)p[r][j].x;
+            for (int r = 0; r < DEFL_RB; ++r) {
+                if (r < nr) {
+                    double re = 0, im = 0;
+#pragma unroll
+                    for (int j = 0; j < PROJ_EPT; ++j) {
+                        if (base + (size_t)j * BLAS_THREADS < n) {
+                            re += (double)f[q][j].x * (double)p[r][j].x + (double)f[q][j].y * (double)p[r][j].y;
+                            im += (double)f[q][j].x * (double)p[r][j].y - (double)f[q][j].y * (double)p[r][j].x;
+                        }
                     }
+                    re = warp_sum(re);
+                    im = warp_sum(im);
+                    if (l == 0) { buf[w][2 * r] = re; buf[w][2 * r + 1] = im; }
                 }
-                re = warp_sum(re);
-                im = warp_sum(im);
-                if (l == 0) { buf[w][2 * r] = re; buf[w][2 * r + 1] = im; }
             }
         }
         __syncthreads();  // (the other half of sm is rewritten only after the next barrier)
-        if (threadIdx.x < nr) {
-            double re = 0, im = 0;
-            for (int q = 0; q < BLAS_THREADS / 32; ++q) { re += buf[q][2 * threadIdx.x]; im += buf[q][2 * threadIdx.x + 1]; }
-            partial[((size_t)(r0 + threadIdx.x) * nev + i) * gridDim.x + blockIdx.x] = make_double2(re, im);
+        if (threadIdx.x < nr * PROJ_IB) {
+            const int q = threadIdx.x / nr, r = threadIdx.x - q * nr;
+            if (i0 + q < nev) {
+                double (*buf)[2 * DEFL_RB] = sm[pass & 1][q];
+                double re = 0, im = 0;
+                for (int k = 0; k < BLAS_THREADS / 32; ++k) { re += buf[k][2 * r]; im += buf[k][2 * r + 1]; }
+                partial[((size_t)(r0 + r) * nev + i0 + q) * gridDim.x + blockIdx.x] = make_double2(re, im);
+            }
         }
     }
 }
