@@ -45,7 +45,8 @@ def rough_alpha(n, seed=5):
     return a
 
 
-DW_DIMS = [(4, 4, 4, 4), (2, 2, 2, 2), (4, 6, 8, 10), (6, 4, 2, 8), (8, 8, 8, 8), (10, 6, 4, 12), (8, 8, 8, 32)]
+# even, extent-2, non-cubic, ragged tiles (V % 128 != 0) and odd extents (the forward and backward wrap of an odd direction differ)
+DW_DIMS = [(4, 4, 4, 4), (2, 2, 2, 2), (4, 6, 8, 10), (6, 4, 2, 8), (8, 8, 8, 8), (10, 6, 4, 12), (8, 8, 8, 32), (3, 5, 4, 6), (5, 3, 7, 3)]
 
 
 @pytest.mark.parametrize("dims", DW_DIMS)
@@ -60,7 +61,7 @@ def test_dw_fp64(torch, api, orc, dims, recon):
     assert np.abs(got - want).max() < 1e-12 * np.abs(want).max() * 10
 
 
-@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (8, 8, 8, 32)])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (8, 8, 8, 32), (5, 3, 7, 3)])
 @pytest.mark.parametrize("recon", [18, 12])
 def test_dw_fp32(torch, api, orc, dims, recon):
     U = inputs.random_links(dims, 0.7, 31)

@@ -37,7 +37,7 @@ def test_gamma_basis_matches_golden_and_clifford(orc):
 
 # ---------------------------------------------------------------- D_W (eq. 2.2)
 
-@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (2, 2, 2, 2), (6, 4, 2, 8)])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (2, 2, 2, 2), (6, 4, 2, 8), (3, 5, 4, 6), (5, 3, 7, 3)])
 def test_dw_free_field_plane_waves(orc, dims):
     """U = 1: D_W u e^{ipx} = [(4 - sum cos p) + i sum gamma sin p] u e^{ipx}; antiperiodic t -> p_t half-integer."""
     gam = golden_gammas()
@@ -74,7 +74,7 @@ def test_dw_free_spectrum_dense(orc):
         assert np.allclose(ev[key(ev)], want[key(want)], atol=1e-9)
 
 
-@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10)])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (5, 3, 7, 3)])
 def test_dw_gamma5_hermiticity(orc, dims):
     """<chi, gamma5 D_W gamma5 psi> = <D_W chi, psi> on rough random links."""
     U = inputs.random_links(dims, 0.9, 5)
@@ -85,7 +85,7 @@ def test_dw_gamma5_hermiticity(orc, dims):
     assert abs(lhs - rhs) / abs(lhs) < 1e-13
 
 
-@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10)])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (5, 3, 7, 3)])
 def test_dw_gauge_covariance(orc, dims):
     """D_W[U^g](g psi) = g D_W[U] psi, U^g_mu(x) = g(x) U_mu(x) g(x+mu)^dag: every link path vs a closed form."""
     U = inputs.random_links(dims, 0.7, 21)
