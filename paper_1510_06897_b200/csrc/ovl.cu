@@ -150,6 +150,12 @@ int create_impl(ovl_ctx **out, const int dims[4], const void *links_c128, int pr
             if (best > 0 && best < dims[2]) { c->sweep.tpc = c->g.sxy * best / 128; c->sweep.nzs = dims[2] / best; }
         }
     }
+    // brick order (ovl_types.cuh): lattices up to 2^18 sites (8^4 ... 16^3 x 32: a launch is bound by the per-SM L2 -> L1 fill
+    // rate; measured -8 ... -15 % per order, neutral from 20^3 x 64 on), Lz and Lt even
+    if (c->g.V <= (1 << 18) && dims[2] % 2 == 0 && dims[3] % 2 == 0) {
+        c->brick.half = c->g.sxyz / 2;
+        c->brick.nchunk = (c->brick.half + ovl::BRICK_GS - 1) / ovl::BRICK_GS;
+    }
     c->prec = prec;
     c->recon = recon;
     c->st = (cudaStream_t)cuda_stream;

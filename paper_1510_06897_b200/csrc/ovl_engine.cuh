@@ -58,6 +58,12 @@ template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx 
             return;
         }
     }
+    if (c->brick.nchunk > 0 && a.nrhs == 1) {
+        static_assert(TH == 4 * BRICK_GS, "brick CTAs are 4 groups of BRICK_GS sites");
+        k_wilson_fused_brick<T, RECON, FLAGS><<<c->brick.nchunk * (c->g.L[3] / 2), TH, 0, c->st>>>(
+            c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp, c->brick);
+        return;
+    }
     if (a.nrhs > 1)
         k_wilson_fused_multi<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
             c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp,

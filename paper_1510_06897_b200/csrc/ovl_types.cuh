@@ -57,6 +57,22 @@ __device__ __forceinline__ int sweep_tile(const Sweep &sw, int Lt, int pos) {
     return (t * sw.nzs + zs) * sw.tpc + w;
 }
 
+// Brick order for lattices small enough that a launch is bound by what every SM pulls out of the L2 (L1 is cold at every
+// launch): a 128-thread CTA handles a 2 x 2 stack in (z, t) of chunks of 32 sites that are consecutive in the half volume
+// u = x + Lx (y + Ly (z / 2)), so the z and t neighbours (and backward links) of half of the hops are the centre sites of
+// another warp of the same CTA and are found in its L1.  Needs Lz and Lt even.  nchunk = 0: plain order.
+struct Brick { int nchunk, half; };
+constexpr int BRICK_GS = 32;
+// CTA index, thread -> site (or -1 for the ragged end of the last chunk of a time-slice pair)
+__device__ __forceinline__ int brick_site(const Brick &bk, const Geom &g, int cta, int thread) {
+    const int grp = thread / BRICK_GS, li = thread - grp * BRICK_GS;
+    const int th = cta / bk.nchunk, ch = cta - th * bk.nchunk;
+    const int u = ch * BRICK_GS + li;
+    if (u >= bk.half) return -1;
+    const int zh = u / g.sxy, r = u - zh * g.sxy;
+    return r + g.sxy * (2 * zh + (grp & 1)) + g.sxyz * (2 * th + (grp >> 1));
+}
+
 // read-only (non-coherent) loads, for the fields a kernel never writes (links, the stencil operand, psi, eigenvectors);
 // `prev` of the fused kernel may alias its output and is NOT read through this path
 __device__ __forceinline__ double2 ldg(const double2 *p) { return __ldg(p); }

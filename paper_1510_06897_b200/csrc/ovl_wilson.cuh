@@ -183,13 +183,11 @@ template <typename T, int THREADS, bool ENABLE> __device__ __forceinline__ cx<T>
     }
 }
 
-// The kernel body for one tile of THREADS consecutive sites of one right-hand side.
+// The kernel body for site s of one right-hand side (THREADS = CTA size: the accumulator staging is indexed by thread).
 template <typename T, int RECON, int FLAGS, int THREADS>
-__device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in,
+__device__ __forceinline__ void wilson_site(const Geom &g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in,
                                             const cx<T> *prev, const cx<T> *__restrict__ psi, cx<T> *out,
-                                            cx<T> *__restrict__ acc, const StepParams<T> &sp, int tile) {
-    const int s = tile * THREADS + threadIdx.x;
-    if (s >= g.V) return;
+                                            cx<T> *__restrict__ acc, const StepParams<T> &sp, const int s) {
     const int x = s % g.L[0];
     const int y = (s / g.L[0]) % g.L[1];
     const int z = (s / g.sxy) % g.L[2];
@@ -258,6 +256,16 @@ __device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restri
     }
 }
 
+// ... for one tile of THREADS consecutive sites
+template <typename T, int RECON, int FLAGS, int THREADS>
+__device__ __forceinline__ void wilson_tile(const Geom &g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in,
+                                            const cx<T> *prev, const cx<T> *__restrict__ psi, cx<T> *out,
+                                            cx<T> *__restrict__ acc, const StepParams<T> &sp, int tile) {
+    const int s = tile * THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    wilson_site<T, RECON, FLAGS, THREADS>(g, U, in, prev, psi, out, acc, sp, s);
+}
+
 // Single right-hand side: the field pointers stay kernel parameters (constant bank).
 template <typename T, int RECON, int FLAGS, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -292,4 +300,16 @@ k_wilson_fused_multi(const Geom g, const cx<T> *__restrict__ U, const cx<T> *in,
                                           (FLAGS & K_NOWRITE) ? out : out + off, (FLAGS & (K_ACC | K_ACCI)) ? acc + off : acc, sp, tile);
 }
 
+// The single-right-hand-side kernel in brick order (Brick, ovl_types.cuh) for small lattices: same arithmetic per site, so
+// the results are bit-identical to the plain order.  4 * BRICK_GS = 128 threads per CTA; such a lattice is at most a few CTAs
+// per SM, so the kernel is compiled without an occupancy target (up to 255 registers, no spills, deeper load batches).
+// (Several right-hand sides stay on k_wilson_fused_multi: with nrhs CTAs per tile the plain order measured faster.)
+template <typename T, int RECON, int FLAGS>
+__global__ void __launch_bounds__(4 * BRICK_GS, 1)
+k_wilson_fused_brick(const Geom g, const cx<T> *__restrict__ U, const cx<T> *__restrict__ in, const cx<T> *prev,
+                     const cx<T> *__restrict__ psi, cx<T> *out, cx<T> *__restrict__ acc, const StepParams<T> sp, const Brick bk) {
+    const int s = brick_site(bk, g, sp.flip ? gridDim.x - 1 - blockIdx.x : blockIdx.x, threadIdx.x);
+    if (s < 0) return;
+    wilson_site<T, RECON, FLAGS, 4 * BRICK_GS>(g, U, in, prev, psi, out, acc, sp, s);
+}
 }  // namespace ovl
