@@ -57,7 +57,7 @@ enum { OVL_F64 = 0, OVL_F32 = 1 };        /* storage + stencil arithmetic precis
 enum { OVL_RECON18 = 18, OVL_RECON12 = 12 }; /* reals stored per link; 12: third row rebuilt as conj(r0 x r1) */
 #define OVL_MAX_RHS 12                        /* right-hand sides per multi call (12 = one propagator's spin-colour sources) */
 enum { OVL_REC_CLENSHAW = 0, OVL_REC_FORWARD = 1 }; /* how sum_m alpha_m T_m(K^) psi of eq. 2.3 is evaluated */
-enum { OVL_FUSED_REGISTER = 0, OVL_FUSED_BULK = 1 }; /* implementation of the fused Wilson / Chebyshev launch */
+enum { OVL_FUSED_REGISTER = 0, OVL_FUSED_BULK = 1, OVL_FUSED_PLAIN = 2 }; /* implementation of the fused Wilson / Chebyshev launch */
 
 /* Library version string, e.g. "ovl-b200 0.1 (sm_100a)". */
 const char *ovl_version(void);
@@ -115,14 +115,19 @@ int ovl_set_recurrence(ovl_ctx *ctx, int mode);
 int ovl_get_recurrence(const ovl_ctx *ctx);
 
 /* Implementation of the fused Wilson-stencil / Chebyshev-step launch ("merging ... into a single GPU kernel";
- * :70-72 on the transfer "from global memory to the registers").  Both give bit-identical results.
+ * :70-72 on the transfer "from global memory to the registers").  All give bit-identical results.
  *   OVL_FUSED_REGISTER  one thread per site, every operand lands in registers through coalesced 128-bit loads (default:
  *                       the faster one on B200 at every size measured);
  *   OVL_FUSED_BULK      persistent warps; the first-touch stream of a warp's own links lands in shared memory by
  *                       cp.async.bulk with mbarrier completion and is refilled for the warp's next 32 sites while the
  *                       current ones are computed.  Used for single-right-hand-side launches of D_W, K^ and the Clenshaw
  *                       recurrence when V and Lx*Ly*Lz are multiples of 32; other launches use the default kernel.
- * Kept selectable so that the comparison (bench.py extras) can be re-measured. */
+ *   OVL_FUSED_PLAIN     the register kernel with the CTAs always in plain site order.  (Under OVL_FUSED_REGISTER a lattice of
+ *                       at most 2^18 sites with Lz and Lt even runs its single-right-hand-side launches in "brick" order: a
+ *                       CTA takes a 2 x 2 stack in (z, t) of 32-site chunks, so half of the z / t neighbours come out of its
+ *                       own L1 -- 8^3 x 32: 5.7 -> 4.9 us per order.  Same arithmetic per site, same bits.)
+ * Kept selectable so that the comparisons (bench.py extras) can be re-measured and the tests can hold every
+ * variant against the others. */
 int ovl_set_fused_variant(ovl_ctx *ctx, int variant);
 
 /* The polynomial loop is a fixed launch sequence per source field; by default it is captured once into a CUDA graph and

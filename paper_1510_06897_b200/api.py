@@ -75,8 +75,9 @@ class Overlap:
         B.ovl_set_recurrence(self.ctx, m)
 
     def set_fused_variant(self, variant):
-        """'register' (default) or 'bulk' (cp.async.bulk landing zone for the links): same results, see include/ovl.h."""
-        v = {"register": B.OVL_FUSED_REGISTER, "bulk": B.OVL_FUSED_BULK}.get(variant, variant)
+        """'register' (default; brick order on small lattices), 'plain' (register kernel, plain site order) or 'bulk' (cp.async.bulk
+        landing zone for the links): same results bit for bit, see include/ovl.h."""
+        v = {"register": B.OVL_FUSED_REGISTER, "bulk": B.OVL_FUSED_BULK, "plain": B.OVL_FUSED_PLAIN}.get(variant, variant)
         B.ovl_set_fused_variant(self.ctx, v)
 
     def set_graphs(self, on=True):

@@ -156,6 +156,7 @@ int create_impl(ovl_ctx **out, const int dims[4], const void *links_c128, int pr
         c->brick.half = c->g.sxyz / 2;
         c->brick.nchunk = (c->brick.half + ovl::BRICK_GS - 1) / ovl::BRICK_GS;
     }
+    c->brick_auto = c->brick;
     c->prec = prec;
     c->recon = recon;
     c->st = (cudaStream_t)cuda_stream;
@@ -338,8 +339,10 @@ int ovl_get_recurrence(const ovl_ctx *c) { return c ? c->recurrence : -1; }
 
 int ovl_set_fused_variant(ovl_ctx *c, int variant) {
     if (!c) return OVL_EINVAL;
-    if (variant != OVL_FUSED_REGISTER && variant != OVL_FUSED_BULK) return fail(c, OVL_EINVAL, "unknown fused-kernel variant %d", variant);
+    if (variant != OVL_FUSED_REGISTER && variant != OVL_FUSED_BULK && variant != OVL_FUSED_PLAIN)
+        return fail(c, OVL_EINVAL, "unknown fused-kernel variant %d", variant);
     c->fused_variant = variant;
+    c->brick = variant == OVL_FUSED_PLAIN ? ovl::Brick{0, 0} : c->brick_auto;
     ++c->poly_gen;  // captured graphs hold the other kernel
     return OVL_OK;
 }
