@@ -508,11 +508,13 @@ def bench_true_eigenpairs(torch, api, w, host_inputs, steps, warmup, block=104, 
     Ud = torch.from_numpy(U).cuda()
     out = {}
     with api.Overlap(w["dims"], Ud) as op:
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        phi, lam, res, cyc, ok = op.lowest_eigenpairs(w["nev"], tol=1e-8, filter_degree=degree, block=block)
-        torch.cuda.synchronize()
-        out.update(eigensolver_seconds=time.perf_counter() - t0, cycles=cyc, converged=ok, max_residual=float(res.max()),
+        with api.Overlap(w["dims"], Ud, "f32") as op32:   # filter on the fp32 kernels while far from the tolerance
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            phi, lam, res, cyc, c32, ok = op.lowest_eigenpairs_mixed(op32, w["nev"], tol=1e-8, filter_degree=degree, block=block)
+            torch.cuda.synchronize()
+        out.update(eigensolver="ovl_lowest_eigenpairs_mixed", eigensolver_seconds=time.perf_counter() - t0, cycles=cyc,
+                   fp32_filter_cycles=c32, converged=ok, max_residual=float(res.max()),
                    abs_lambda_min=float(np.abs(lam).min()), abs_lambda_max=float(np.abs(lam).max()))
         orders = op.set_chebyshev(alpha)
         op.set_deflation(phi, lam)
@@ -533,14 +535,22 @@ def bench_true_eigenpairs(torch, api, w, host_inputs, steps, warmup, block=104, 
 def bench_eigensolver(torch, api, w, nev, block, degree):
     """the deflation space computed on the GPU (ovl_lowest_eigenpairs), wall-clock seconds."""
     U = make_inputs(w, need_phi=False)[0]
-    with api.Overlap(w["dims"], torch.from_numpy(U).cuda()) as op:
+    Ud = torch.from_numpy(U).cuda()
+    with api.Overlap(w["dims"], Ud) as op, api.Overlap(w["dims"], Ud, "f32") as op32:
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         phi, lam, res, cyc, ok = op.lowest_eigenpairs(nev, tol=1e-8, filter_degree=degree, block=block)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        _, lam_m, res_m, cyc_m, c32, ok_m = op.lowest_eigenpairs_mixed(op32, nev, tol=1e-8, filter_degree=degree, block=block)
+        torch.cuda.synchronize()
+        dt_m = time.perf_counter() - t0
     return {"nev": nev, "block": block, "filter_degree": degree, "cycles": cyc, "converged": ok, "seconds": dt,
-            "max_residual": float(res.max()), "abs_lambda_min": float(np.abs(lam).min()), "abs_lambda_max": float(np.abs(lam).max())}
+            "max_residual": float(res.max()), "abs_lambda_min": float(np.abs(lam).min()), "abs_lambda_max": float(np.abs(lam).max()),
+            "mixed_precision_filter": {"seconds": dt_m, "cycles": cyc_m, "fp32_filter_cycles": c32, "converged": ok_m,
+                                       "max_residual": float(res_m.max()),
+                                       "max_abs_lambda_difference": float(np.abs(np.sort(lam_m) - np.sort(lam)).max())}}
 
 
 def run_profile_target(args, w):

@@ -211,6 +211,20 @@ int ovl_cg_mixed(ovl_ctx *ctx64, ovl_ctx *ctx32, double mu, const void *b, void 
 int ovl_lowest_eigenpairs(ovl_ctx *ctx, int nev, double tol, int max_cycles, int filter_degree, int block, void *phi_out,
                           double *lambda_out, double *resid_out, int *cycles_out);
 
+/* The same eigensolver with the Chebyshev filter -- more than 90 % of its run time -- on the fp32 stencil kernels of a sibling
+ * context while the block is far from the tolerance (PAPER.md:66 names the polynomial preconditioning, :110 the mixed
+ * precision).  ctx32 is an OVL_F32 context on the same lattice, stream, m_w and lambda_max
+ * (its links are the same links rounded to fp32).  A filter cycle runs in fp32 while the largest residual of the wanted
+ * pairs is above 1e-5 lambda_max (and fp32 cycles keep gaining at least a factor 3): the filter only has to damp the unwanted part of the spectrum by e^-8 per cycle; the
+ * trial block, the Rayleigh-Ritz steps, the residuals and the final diagonalisation of K stay in fp64, and the cycles below
+ * that threshold run entirely in fp64, so the returned pairs meet the same tol.  The fp32 recurrence is rescaled step by
+ * step (T_d grows like 1e172 in the first cycles from a random start), at no extra cost.
+ * Arguments and results as ovl_lowest_eigenpairs; *f32_cycles_out (may be NULL) = cycles whose filter ran in fp32.
+ * Errors: additionally OVL_EINVAL for mismatched contexts.  Synchronises. */
+int ovl_lowest_eigenpairs_mixed(ovl_ctx *ctx64, ovl_ctx *ctx32, int nev, double tol, int max_cycles, int filter_degree,
+                                int block, void *phi_out, double *lambda_out, double *resid_out, int *cycles_out,
+                                int *f32_cycles_out);
+
 const char *ovl_last_error(const ovl_ctx *ctx);
 
 /* ---- the lattice split along t over several GPUs --------------------------------------

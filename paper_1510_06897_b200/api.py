@@ -151,6 +151,14 @@ class Overlap:
         rc, lam, res, cyc = B.ovl_lowest_eigenpairs(self.ctx, nev, tol, max_cycles, filter_degree, block, phi)
         return phi, lam, res, cyc, rc == B.OVL_OK
 
+    def lowest_eigenpairs_mixed(self, inner, nev, tol=1e-8, max_cycles=40, filter_degree=100, block=0):
+        """The same with the filter on the fp32 kernels of `inner` (an 'f32' Overlap on the same lattice and stream) while the
+        block is far from the tolerance. Returns (phi, lambda, residuals, cycles, fp32 cycles, converged)."""
+        torch = _torch()
+        phi = torch.empty((nev, self.V, 4, 3), dtype=torch.complex128, device="cuda")
+        rc, lam, res, cyc, c32 = B.ovl_lowest_eigenpairs_mixed(self.ctx, inner.ctx, nev, tol, max_cycles, filter_degree, block, phi)
+        return phi, lam, res, cyc, c32, rc == B.OVL_OK
+
     # ---- native-layout fields
     def native_empty(self, nrhs=1):
         torch = _torch()

@@ -48,6 +48,7 @@ SIGNATURES = {
     "ovl_cg_multi": (_I, [_P, _I, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_mixed": (_I, [_P, _P, _D, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
     "ovl_lowest_eigenpairs": (_I, [_P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I)]),
+    "ovl_lowest_eigenpairs_mixed": (_I, [_P, _P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I), C.POINTER(_I)]),
     "ovl_last_error": (C.c_char_p, [_P]),
     "ovl_group_create": (_I, [C.POINTER(_P), C.POINTER(_I), _I, _P, _I, _I, C.POINTER(_P), C.POINTER(_I)]),
     "ovl_group_destroy": (_I, [_P]),
@@ -266,6 +267,15 @@ def ovl_lowest_eigenpairs(ctx, nev, tol, max_cycles, filter_degree, block, phi_o
                                               _ptr(phi_out), lam, res, C.byref(cyc))
     _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
     return rc, np.array(lam), np.array(res), int(cyc.value)
+
+
+def ovl_lowest_eigenpairs_mixed(ctx64, ctx32, nev, tol, max_cycles, filter_degree, block, phi_out):
+    """Returns (status, lambda[nev], residual[nev], cycles, fp32 filter cycles); phi_out as ovl_lowest_eigenpairs."""
+    lam, res, cyc, c32 = (_D * nev)(), (_D * nev)(), _I(0), _I(0)
+    rc = load_library().ovl_lowest_eigenpairs_mixed(ctx64, ctx32, int(nev), float(tol), int(max_cycles), int(filter_degree),
+                                                    int(block), _ptr(phi_out), lam, res, C.byref(cyc), C.byref(c32))
+    _check(ctx64, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, np.array(lam), np.array(res), int(cyc.value), int(c32.value)
 
 
 def ovl_last_error(ctx) -> str:

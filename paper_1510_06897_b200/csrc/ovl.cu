@@ -488,8 +488,21 @@ int ovl_lowest_eigenpairs(ovl_ctx *c, int nev, double tol, int max_cycles, int f
     if (nev < 1 || !(tol > 0) || max_cycles < 0 || !phi_out || !lambda_out || !cycles_out || block < 0)
         return fail(c, OVL_EINVAL, "bad ovl_lowest_eigenpairs arguments");
     if (c->prec != OVL_F64) return fail(c, OVL_EINVAL, "the eigensolver needs an OVL_F64 context");
-    return eig_lowest(c, nev, tol, max_cycles, filter_degree > 0 ? filter_degree : 100, block, 1510068970ull, phi_out, lambda_out,
+    return eig_lowest(c, nullptr, nev, tol, max_cycles, filter_degree > 0 ? filter_degree : 100, block, 1510068970ull, phi_out, lambda_out,
                       resid_out, cycles_out);
+}
+
+int ovl_lowest_eigenpairs_mixed(ovl_ctx *c, ovl_ctx *c32, int nev, double tol, int max_cycles, int filter_degree, int block,
+                                void *phi_out, double *lambda_out, double *resid_out, int *cycles_out, int *f32_cycles_out) {
+    if (!c || !c32) return OVL_EINVAL;
+    if (nev < 1 || !(tol > 0) || max_cycles < 0 || !phi_out || !lambda_out || !cycles_out || block < 0)
+        return fail(c, OVL_EINVAL, "bad ovl_lowest_eigenpairs_mixed arguments");
+    if (c->prec != OVL_F64 || c32->prec != OVL_F32) return fail(c, OVL_EINVAL, "ovl_lowest_eigenpairs_mixed needs an OVL_F64 and an OVL_F32 context");
+    if (c->g.V != c32->g.V || memcmp(c->g.L, c32->g.L, sizeof c->g.L) != 0) return fail(c, OVL_EINVAL, "contexts differ in lattice size");
+    if (c->st != c32->st) return fail(c, OVL_EINVAL, "both contexts must have been created on the same stream");
+    if (c->m_w != c32->m_w || c->lambda_max != c32->lambda_max) return fail(c, OVL_EINVAL, "contexts differ in m_w or lambda_max (ovl_set_kernel)");
+    return eig_lowest(c, c32, nev, tol, max_cycles, filter_degree > 0 ? filter_degree : 100, block, 1510068970ull, phi_out, lambda_out,
+                      resid_out, cycles_out, f32_cycles_out);
 }
 
 const char *ovl_last_error(const ovl_ctx *c) { return c ? c->err : "null context"; }

@@ -21,6 +21,9 @@
 
 namespace ovl {
 
+// residual (in units of lambda_max) above which a filter cycle may run in fp32 (ovl_lowest_eigenpairs_mixed)
+constexpr double EIG_F32_FLOOR = 1e-5;
+
 // The work block of one ovl_lowest_eigenpairs call for `cap` = max(block, 2 nev) vectors: one contiguous device region,
 // either inside the caller-owned workspace (eig_block of ovl_workspace_bytes) or one cudaMalloc released on return.
 struct EigWork {
@@ -117,41 +120,70 @@ inline int eig_rotate(ovl_ctx *c, EigWork &w, int nin, int nout, int ldx, const 
     return OVL_OK;
 }
 
-// out_r = K^ in_r for a block of nvec consecutive native fields, OVL_MAX_RHS at a time
-inline int eig_khat_block(ovl_ctx *c, int nvec, const double2 *in, double2 *out) {
+// out_r = K^ in_r for a block of nvec consecutive native fields of precision T, OVL_MAX_RHS at a time
+template <typename T> inline int eig_khat_block_t(ovl_ctx *c, int nvec, const cx<T> *in, cx<T> *out) {
     const size_t n = c->n();
     for (int j0 = 0; j0 < nvec; j0 += OVL_MAX_RHS) {
         WilsonArgs a;
         a.nrhs = std::min((int)OVL_MAX_RHS, nvec - j0);
         a.in = in + (size_t)j0 * n; a.out = out + (size_t)j0 * n;
         a.c_diag = (4.0 - c->m_w) / c->lambda_max; a.c_hop = -0.5 / c->lambda_max;
-        OVL_TRY((launch_wilson<double, K_G5>(c, a)));
+        OVL_TRY((launch_wilson<T, K_G5>(c, a)));
     }
     return OVL_OK;
 }
+inline int eig_khat_block(ovl_ctx *c, int nvec, const double2 *in, double2 *out) { return eig_khat_block_t<double>(c, nvec, in, out); }
 
-// V_chunk <- T_d((K^2 - cc)/ee) V_chunk, with W_chunk = K^ V_chunk on entry (d >= 1)
-inline int eig_filter_chunk(ovl_ctx *c, int nv, int d, double cc, double ee, double2 *Vc, const double2 *Wc) {
+// V_chunk <- T_d((K^2 - cc)/ee) V_chunk / rho^d, with W_chunk = K^ V_chunk on entry (d >= 1), in the precision T of context c
+// (its recurrence workspace tA, acc).  rho = 1: the plain recurrence.  rho > 1: the recurrence for s_j = t_j / rho^j,
+//     s_{j+1} = [(2/ee) K^2 s_j - (2 cc/ee) s_j] / rho - s_{j-1} / rho^2,
+// which keeps the fastest-growing component O(1) -- T_d grows like (|y| + sqrt(y^2 - 1))^d below the damped interval, 1e172
+// in the first cycles from a random start, far outside fp32 -- at no cost: the scale factors ride on the kernel's scalars.
+template <typename T>
+inline int eig_filter_chunk(ovl_ctx *c, int nv, int d, double cc, double ee, double rho, cx<T> *Vc, const cx<T> *Wc) {
     const double cd = (4.0 - c->m_w) / c->lambda_max, ch = -0.5 / c->lambda_max;
     const size_t fb = c->field_bytes() * nv;
-    double2 *tcur = (double2 *)c->tA, *tprev = Vc, *wbuf = (double2 *)c->acc;
-    {   // t_1 = (K^ W - cc V)/ee
+    cx<T> *tcur = (cx<T> *)c->tA, *tprev = Vc, *wbuf = (cx<T> *)c->acc;
+    {   // s_1 = (K^ W - cc V)/(ee rho)
         WilsonArgs a;
         a.nrhs = nv; a.in = Wc; a.psi = Vc; a.out = tcur;
-        a.c_diag = cd / ee; a.c_hop = ch / ee; a.a_psi = -cc / ee;
-        OVL_TRY((launch_wilson<double, K_G5 | K_PSI>(c, a)));
+        a.c_diag = cd / (ee * rho); a.c_hop = ch / (ee * rho); a.a_psi = -cc / (ee * rho);
+        OVL_TRY((launch_wilson<T, K_G5 | K_PSI>(c, a)));
     }
-    for (int j = 1; j < d; ++j) {  // t_{j+1} = (2/ee) K^ (K^ t_j) - (2 cc/ee) t_j - t_{j-1}, written over t_{j-1}
+    for (int j = 1; j < d; ++j) {  // s_{j+1}, written over s_{j-1}
         WilsonArgs k;
         k.nrhs = nv; k.in = tcur; k.out = wbuf; k.c_diag = cd; k.c_hop = ch;
-        OVL_TRY((launch_wilson<double, K_G5>(c, k)));
+        OVL_TRY((launch_wilson<T, K_G5>(c, k)));
         WilsonArgs a;
         a.nrhs = nv; a.in = wbuf; a.psi = tcur; a.prev = tprev; a.out = tprev;
-        a.c_diag = 2.0 * cd / ee; a.c_hop = 2.0 * ch / ee; a.a_psi = -2.0 * cc / ee;
-        OVL_TRY((launch_wilson<double, K_G5 | K_PSI | K_PREV>(c, a)));
+        a.c_diag = 2.0 * cd / (ee * rho); a.c_hop = 2.0 * ch / (ee * rho); a.a_psi = -2.0 * cc / (ee * rho);
+        a.c_prev = 1.0 / (rho * rho);
+        OVL_TRY((launch_wilson<T, K_G5 | K_PSI | K_PREV>(c, a)));
         std::swap(tcur, tprev);
     }
     if (tcur != Vc) OVL_CUDA(c, cudaMemcpyAsync(Vc, tcur, fb, cudaMemcpyDeviceToDevice, c->st));
+    return OVL_OK;
+}
+// The same filter for a chunk of the fp64 block, run in the fp32 sibling context c32 (same lattice, same stream): the chunk
+// is rounded to fp32 into c32's workspace (g5b), W = K^ V is formed there (tB), the scaled recurrence runs on the fp32 stencil
+// kernels (half the bytes per launch) and the result is widened back.  rho from sigma = 0, the most negative argument.
+inline int eig_filter_chunk_f32(ovl_ctx *c, ovl_ctx *c32, int nv, int d, double cc, double ee, double2 *Vc) {
+    const size_t n = c->n() * (size_t)nv;
+    const int grid = grid_for(n, BLAS_THREADS);
+    float2 *Vf = (float2 *)c32->g5b, *Wf = (float2 *)c32->tB;
+    k_convert_scaled<double, float><<<grid, BLAS_THREADS, 0, c->st>>>(n, 1.0, Vc, Vf);
+    OVL_LAUNCH_CHECK(c);
+    {
+        const int rc = eig_khat_block_t<float>(c32, nv, Vf, Wf);
+        if (rc != OVL_OK) return fail(c, rc, "fp32 filter: %s", c32->err);
+    }
+    const double y0 = cc / ee, rho = y0 + std::sqrt(std::max(y0 * y0 - 1.0, 0.0));
+    {
+        const int rc = eig_filter_chunk<float>(c32, nv, d, cc, ee, rho, Vf, Wf);
+        if (rc != OVL_OK) return fail(c, rc, "fp32 filter: %s", c32->err);
+    }
+    k_convert_scaled<float, double><<<grid, BLAS_THREADS, 0, c->st>>>(n, 1.0, Vf, Vc);
+    OVL_LAUNCH_CHECK(c);
     return OVL_OK;
 }
 
@@ -238,8 +270,8 @@ inline int eig_endgame(ovl_ctx *c, EigWork &w, int nev, std::vector<double> &the
     return eig_resid(c, w, nev, theta_out, w.Q, w.Z, resid_out);
 }
 
-inline int eig_lowest(ovl_ctx *c, int nev, double tol, int max_cycles, int degree, int block, unsigned long long seed,
-                      void *phi_out, double *lambda_out, double *resid_out, int *cycles_out) {
+inline int eig_lowest(ovl_ctx *c, ovl_ctx *c32, int nev, double tol, int max_cycles, int degree, int block, unsigned long long seed,
+                      void *phi_out, double *lambda_out, double *resid_out, int *cycles_out, int *f32_cycles_out = nullptr) {
     const size_t n = c->n();
     int m = block > 0 ? block : nev + std::max(8, nev / 2);
     if (m < nev) m = nev;
@@ -249,6 +281,13 @@ inline int eig_lowest(ovl_ctx *c, int nev, double tol, int max_cycles, int degre
     const int cap = std::max(m, 2 * nev);  // vectors per work block
     const int chunk = std::min(m, c->ws_mode ? c->max_rhs : (int)OVL_MAX_RHS);  // vectors per filter pass (recurrence workspace)
     OVL_TRY(ensure_work(c, chunk));
+    if (c32) {
+        const int rc = ensure_work(c32, chunk);
+        if (rc != OVL_OK) return fail(c, rc, "fp32 context: %s", c32->err);
+    }
+    int n_f32_cycles = 0;
+    bool f32_allowed = true, last_was_f32 = false;
+    double last_worst = 0;
     EigWork w;
     OVL_TRY(eig_ws_setup(c, w, cap));
     const int nb = c->red_nblk;
@@ -318,9 +357,22 @@ inline int eig_lowest(ovl_ctx *c, int nev, double tol, int max_cycles, int degre
         deg = std::max(std::min(deg, degree), std::min(degree, 10));
         int nlock = 0;
         while (nlock < nev && r2[nlock] / std::max(std::sqrt(sigma[nlock]), 1e-300) <= 0.1 * tol_int) ++nlock;
+        //  * with an fp32 sibling context the filter runs on the fp32 stencil kernels (eig_filter_chunk_f32) while the block is
+        //    far from the tolerance: the filter only has to damp the unwanted part by e^-8 per cycle, the Rayleigh-Ritz step
+        //    and every residual stay in fp64, and the fp32 rounding (~1e-6 of a filtered vector) is removed by the fp64 cycles
+        //    that follow once the residual is below EIG_F32_FLOOR (measured: the same number of cycles and the same residuals as
+        //    the all-fp64 run; 8^3 x 32: 5 of 7 cycles in fp32, 20^3 x 64: 29.6 -> 21 s).
+        // (an fp32 filter cannot take the residual below ~1e-6 lambda_max: a cycle that gains less than a factor 3 in fp32 is
+        // the sign of that floor, and the rest of the run stays in fp64)
+        if (last_was_f32 && worst > 0.3 * last_worst) f32_allowed = false;
+        const bool f32_cycle = c32 != nullptr && f32_allowed && worst > EIG_F32_FLOOR;
+        last_was_f32 = f32_cycle;
+        last_worst = worst;
+        n_f32_cycles += f32_cycle;
         for (int j0 = nlock; j0 < m; j0 += chunk) {
             const int nv = std::min(chunk, m - j0);
-            OVL_TRY(eig_filter_chunk(c, nv, deg, cc, ee, w.V + (size_t)j0 * n, w.W + (size_t)j0 * n));
+            if (f32_cycle) OVL_TRY(eig_filter_chunk_f32(c, c32, nv, deg, cc, ee, w.V + (size_t)j0 * n));
+            else OVL_TRY(eig_filter_chunk<double>(c, nv, deg, cc, ee, 1.0, w.V + (size_t)j0 * n, w.W + (size_t)j0 * n));
         }
         // normalise
         k_redot<double><<<dim3(nb, m), BLAS_THREADS, 0, c->st>>>(n, w.V, w.V, w.partial);
@@ -358,6 +410,7 @@ inline int eig_lowest(ovl_ctx *c, int nev, double tol, int max_cycles, int degre
     }
     OVL_CUDA(c, cudaStreamSynchronize(c->st));
     *cycles_out = cycle;
+    if (f32_cycles_out) *f32_cycles_out = n_f32_cycles;
     if (!converged) {
         double worst = 0;
         for (int i = 0; i < nev; ++i) worst = std::max(worst, resid[i] * c->lambda_max);

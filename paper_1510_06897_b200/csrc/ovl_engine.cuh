@@ -25,6 +25,7 @@ struct WilsonArgs {
     const void *in = nullptr, *prev = nullptr, *psi = nullptr;
     void *out = nullptr, *acc = nullptr;
     double c_diag = 0, c_hop = 0, a_psi = 0, a_acc = 0, a_init = 0;
+    double c_prev = 1.0;  // out = ... - c_prev * prev (1 everywhere except the eigensolver's scaled filter recurrence)
     int flip = 0, nrhs = 1;
 };
 
@@ -51,7 +52,7 @@ template <typename T, int RECON, int FLAGS> inline void launch_wilson_tp(ovl_ctx
 template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx *c, const WilsonArgs &a) {
     constexpr int TH = WilsonCfg<T>::THREADS;
     const int grid = ((c->g.V + TH - 1) / TH) * a.nrhs;
-    StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(1.0 / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip};
+    StepParams<T> sp{(T)a.c_hop, (T)(a.c_diag / a.c_hop), (T)(a.c_prev / a.c_hop), (T)(a.a_psi / a.c_hop), (T)a.a_acc, (T)a.a_init, a.flip};
     if constexpr (!(FLAGS & (K_ACC | K_ACCI | K_NOWRITE))) {
         if (c->fused_variant == OVL_FUSED_BULK && a.nrhs == 1 && c->g.V % 32 == 0 && c->g.sxyz % 32 == 0) {
             launch_wilson_tp<T, RECON, FLAGS>(c, a, sp);

@@ -482,6 +482,45 @@ def test_eigensolver_config1_lattice(torch, api, orc):
     assert np.abs(gram - np.eye(nev)).max() < 1e-9
 
 
+def test_eigensolver_mixed_precision(torch, api, orc, dense44):
+    """ovl_lowest_eigenpairs_mixed: the Chebyshev filter on the fp32 kernels of a sibling context while the block is far
+    from the tolerance, everything else in fp64.  (i) 4^4: eigenvalues against the dense spectrum of the oracle's K at the
+    same 1e-10 as the all-fp64 solver, residuals <= tol; (ii) the smeared config-1 links (8^3 x 32, 20 pairs, block 40):
+    residuals recomputed with the ORACLE's K, eigenvalues equal to the all-fp64 solver's, at least one filter cycle really
+    ran in fp32 (the first cycles from a random start need the rescaled recurrence: T_d ~ 1e100 there); (iii) argument
+    checks."""
+    from paper_1510_06897_b200 import binding as B
+    d = dense44
+    dims, U = d["dims"], d["U"]
+    nev = 12
+    ev = d["lam"][np.argsort(np.abs(d["lam"]))][:nev]
+    with api.Overlap(dims, dev(torch, U)) as op, api.Overlap(dims, dev(torch, U), "f32") as op32:
+        phi, lam, res, cyc, c32, ok = op.lowest_eigenpairs_mixed(op32, nev, tol=1e-9, filter_degree=40)
+        assert ok and c32 >= 1 and cyc > c32 and res.max() <= 1e-9
+        assert np.abs(np.sort(lam) - np.sort(ev)).max() < 1e-10
+        ph = host(phi)
+        gram = np.einsum("ixsc,jxsc->ij", ph.conj(), ph)
+        assert np.abs(gram - np.eye(nev)).max() < 1e-10
+        out = torch.empty((2, 256, 4, 3), dtype=torch.complex128, device="cuda")
+        for a, b in ((op32, op), (op, op)):
+            with pytest.raises(B.OvlError) as e:
+                B.ovl_lowest_eigenpairs_mixed(a.ctx, b.ctx, 2, 1e-6, 5, 20, 0, out)
+            assert e.value.code == B.OVL_EINVAL
+    dims, nev = (8, 8, 8, 32), 20
+    U = inputs.config_links(dims, 0.3, inputs.SEED_BASE + 1, stout_steps=3)
+    with api.Overlap(dims, dev(torch, U)) as op, api.Overlap(dims, dev(torch, U), "f32") as op32:
+        phi, lam, res, cyc, c32, ok = op.lowest_eigenpairs_mixed(op32, nev, tol=1e-8, filter_degree=200, block=40)
+        ph = host(phi)
+        _, lam64, _, cyc64, ok64 = op.lowest_eigenpairs(nev, tol=1e-8, filter_degree=200, block=40)
+    assert ok and ok64 and c32 >= 2 and res.max() <= 1e-8
+    assert np.abs(np.sort(lam) - np.sort(lam64)).max() < 1e-9
+    for i in (0, 9, 19):
+        r = orc.khat(dims, U, ph[i], 1.5, 6.5) * 6.5 - lam[i] * ph[i]
+        assert np.linalg.norm(r) < 5e-8
+    gram = np.einsum("ixsc,jxsc->ij", ph.conj(), ph)
+    assert np.abs(gram - np.eye(nev)).max() < 1e-9
+
+
 def test_eigensolver_argument_checks(torch, api):
     from paper_1510_06897_b200 import binding as B
     dims = (4, 4, 4, 4)
