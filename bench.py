@@ -495,8 +495,14 @@ def bench_cg_mixed(torch, api, w, host_inputs=None, tol=1e-8, inner_tol=1e-4, la
         torch.cuda.synchronize()
         dt64 = time.perf_counter() - t0
         diff = float(torch.linalg.norm(x - x64) / torch.linalg.norm(x64))
+        # the same in one chirality sector (ovl_cg_mixed_chiral: one sign application per operator application)
+        t0 = time.perf_counter()
+        xc, noc, nic, relc, okc = op.cg_mixed_chiral(op32, bd, 0.05, +1, tol=tol, inner_tol=inner_tol)
+        torch.cuda.synchronize()
+        dtc = time.perf_counter() - t0
     return {"workload": label, "mixed_seconds": dt, "outer_steps": no, "fp32_iterations": ni, "true_relres": rel, "converged": ok,
-            "fp64_seconds": dt64, "fp64_iterations": it64, "fp64_true_relres": rel64, "rel_diff_of_solutions": diff}
+            "fp64_seconds": dt64, "fp64_iterations": it64, "fp64_true_relres": rel64, "rel_diff_of_solutions": diff,
+            "mixed_chiral_sector": {"seconds": dtc, "outer_steps": noc, "fp32_iterations": nic, "true_relres": relc, "converged": okc}}
 
 
 def bench_true_eigenpairs(torch, api, w, host_inputs, steps, warmup, block=104, degree=200):

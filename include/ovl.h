@@ -197,6 +197,14 @@ int ovl_cg_multi(ovl_ctx *ctx, int nrhs, double mu, const void *b, void *x, doub
 int ovl_cg_mixed(ovl_ctx *ctx64, ovl_ctx *ctx32, double mu, const void *b, void *x, double tol, double inner_tol,
                  int max_outer, int max_inner, int *outer_out, int *inner_total_out, double *true_relres_out);
 
+/* ovl_cg_mixed in one chirality sector: the system A_c x = P_c b of ovl_cg_chiral (reading R23; SURVEY.md §8(f)
+ * ranks 2 and 4 combined) by defect correction with fp32 inner solves -- one sign application per operator application in
+ * both precisions.  The outer residual is P_c b - A_c x in fp64.  Arguments, outputs and errors as ovl_cg_mixed;
+ * OVL_EINVAL for chirality not +-1.  x = P_c x.  Synchronises. */
+int ovl_cg_mixed_chiral(ovl_ctx *ctx64, ovl_ctx *ctx32, double mu, int chirality, const void *b, void *x, double tol,
+                        double inner_tol, int max_outer, int max_inner, int *outer_out, int *inner_total_out,
+                        double *true_relres_out);
+
 /* The nev eigenpairs of K = gamma5 (D_W - m_w) of smallest |lambda| -- the deflation space of eq. 2.3 (PAPER.md:62, :66:
  * "a polynomial preconditioned implicitly restarted Lanczos routine"; here a Chebyshev-filtered block subspace iteration on
  * K^2 with a Rayleigh-Ritz step on K, which separates +lambda from -lambda).  OVL_F64 contexts.

@@ -143,6 +143,13 @@ class Overlap:
         rc, no, ni, rel = B.ovl_cg_mixed(self.ctx, inner.ctx, mu, b, x, tol, inner_tol, max_outer, max_inner)
         return x, no, ni, rel, rc == B.OVL_OK
 
+    def cg_mixed_chiral(self, inner, b, mu, chirality, tol=1e-8, inner_tol=1e-4, max_outer=20, max_inner=1000):
+        """cg_mixed on the chirality sector (A_c x = P_c b, one sign application per operator application).
+        Returns (x, outer steps, fp32 iterations, true fp64 relres, converged)."""
+        x = self._like(b)
+        rc, no, ni, rel = B.ovl_cg_mixed_chiral(self.ctx, inner.ctx, mu, chirality, b, x, tol, inner_tol, max_outer, max_inner)
+        return x, no, ni, rel, rc == B.OVL_OK
+
     def lowest_eigenpairs(self, nev, tol=1e-8, max_cycles=40, filter_degree=100, block=0):
         """Deflation space on the GPU: the nev lowest-|lambda| eigenpairs of K. Returns (phi (nev,V,4,3) complex128 CUDA
         tensor, lambda, residuals, cycles, converged)."""

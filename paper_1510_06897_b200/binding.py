@@ -47,6 +47,7 @@ SIGNATURES = {
     "ovl_cg_chiral": (_I, [_P, _D, _I, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_multi": (_I, [_P, _I, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_mixed": (_I, [_P, _P, _D, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_cg_mixed_chiral": (_I, [_P, _P, _D, _I, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
     "ovl_lowest_eigenpairs": (_I, [_P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I)]),
     "ovl_lowest_eigenpairs_mixed": (_I, [_P, _P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I), C.POINTER(_I)]),
     "ovl_last_error": (C.c_char_p, [_P]),
@@ -256,6 +257,15 @@ def ovl_cg_mixed(ctx64, ctx32, mu, b, x, tol, inner_tol, max_outer, max_inner):
     no, ni, rel = _I(0), _I(0), _D(0.0)
     rc = load_library().ovl_cg_mixed(ctx64, ctx32, float(mu), _ptr(b), _ptr(x), float(tol), float(inner_tol), int(max_outer),
                                      int(max_inner), C.byref(no), C.byref(ni), C.byref(rel))
+    _check(ctx64, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, int(no.value), int(ni.value), float(rel.value)
+
+
+def ovl_cg_mixed_chiral(ctx64, ctx32, mu, chirality, b, x, tol, inner_tol, max_outer, max_inner):
+    """Returns (status, outer steps, total fp32 iterations, true fp64 relative residual of the sector system)."""
+    no, ni, rel = _I(0), _I(0), _D(0.0)
+    rc = load_library().ovl_cg_mixed_chiral(ctx64, ctx32, float(mu), int(chirality), _ptr(b), _ptr(x), float(tol), float(inner_tol),
+                                            int(max_outer), int(max_inner), C.byref(no), C.byref(ni), C.byref(rel))
     _check(ctx64, rc, ok=(OVL_OK, OVL_ENOTCONV))
     return rc, int(no.value), int(ni.value), float(rel.value)
 

@@ -482,6 +482,25 @@ int ovl_cg_mixed(ovl_ctx *c, ovl_ctx *c32, double mu, const void *b, void *x, do
     return rc;
 }
 
+int ovl_cg_mixed_chiral(ovl_ctx *c, ovl_ctx *c32, double mu, int chirality, const void *b, void *x, double tol, double inner_tol,
+                        int max_outer, int max_inner, int *outer_out, int *inner_out, double *relres_out) {
+    if (!c || !c32) return OVL_EINVAL;
+    if (!b || !x || b == x || !outer_out || !inner_out || !relres_out || max_outer < 0 || max_inner < 1 || !(tol > 0) || !(inner_tol > 0) ||
+        (chirality != 1 && chirality != -1))
+        return fail(c, OVL_EINVAL, "bad ovl_cg_mixed_chiral arguments (chirality must be +1 or -1)");
+    if (c->prec != OVL_F64 || c32->prec != OVL_F32) return fail(c, OVL_EINVAL, "ovl_cg_mixed_chiral needs an OVL_F64 and an OVL_F32 context");
+    if (c->g.V != c32->g.V || memcmp(c->g.L, c32->g.L, sizeof c->g.L) != 0) return fail(c, OVL_EINVAL, "contexts differ in lattice size");
+    if (c->st != c32->st) return fail(c, OVL_EINVAL, "both contexts must have been created on the same stream");
+    if (c->alpha.empty() || c32->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called on both contexts");
+    OVL_TRY(import_any(c, b, c->psi_n));
+    int rc = cg_mixed_native(c, c32, mu, c->psi_n, c->out_n, tol, inner_tol, max_outer, max_inner, outer_out, inner_out, relres_out, chirality);
+    if (rc != OVL_OK && rc != OVL_ENOTCONV) return rc;
+    int rc2 = export_any(c, c->out_n, x);
+    if (rc2 != OVL_OK) return rc2;
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    return rc;
+}
+
 int ovl_lowest_eigenpairs(ovl_ctx *c, int nev, double tol, int max_cycles, int filter_degree, int block, void *phi_out,
                           double *lambda_out, double *resid_out, int *cycles_out) {
     if (!c) return OVL_EINVAL;

@@ -428,12 +428,19 @@ int cg_native(ovl_ctx *c, double mu, const void *b_n, void *x_n, double tol, int
 // defect correction x <- x + A32^{-1} (b - A64 x).  Outer residuals and the solution are fp64 (context c), the inner
 // solves run the whole fp32 path (context c32: fp32 links, eigenvectors, stencil arithmetic; its own Chebyshev table, which
 // may be of lower degree) on the residual normalised to unit length.  b_n, x_n: native fp64 fields of c.
+// chir = +1 / -1: the chiral-sector system A_c x = P_c b of cg_native (one sign application per operator application in
+// both precisions); the outer residual is P_c b - A_c x.
 inline int cg_mixed_native(ovl_ctx *c, ovl_ctx *c32, double mu, const void *b_n, void *x_n, double tol, double inner_tol,
-                           int max_outer, int max_inner, int *outer_out, int *inner_out, double *relres) {
-    const size_t n = c->n(), fb = c->field_bytes();
+                           int max_outer, int max_inner, int *outer_out, int *inner_out, double *relres, int chir = 0) {
+    const size_t n = c->n(), fb = c->field_bytes(), n_upper = (size_t)6 * c->g.V;
     OVL_TRY(ensure_cg(c, 1));
     const int gridv = grid_for(n, BLAS_THREADS);
     OVL_CUDA(c, cudaMemsetAsync(x_n, 0, fb, c->st));
+    if (chir) {  // P_c b lives in cg_p (the outer iteration has no search direction of its own)
+        k_chiral_project<double><<<dim3(grid_for(n, BLAS_THREADS, 1 << 30), 1), BLAS_THREADS, 0, c->st>>>(n, n_upper, chir, (const double2 *)b_n, (double2 *)c->cg_p);
+        OVL_LAUNCH_CHECK(c);
+        b_n = c->cg_p;
+    }
     OVL_CUDA(c, cudaMemcpyAsync(c->cg_r, b_n, fb, cudaMemcpyDeviceToDevice, c->st));
     OVL_TRY(reduce_redot<double>(c, b_n, b_n, 0, 1));
     OVL_TRY(fetch_scalars(c, 1));
@@ -446,14 +453,18 @@ inline int cg_mixed_native(ovl_ctx *c, ovl_ctx *c32, double mu, const void *b_n,
         OVL_LAUNCH_CHECK(c);
         int it = 0;
         double rel32 = 0;
-        const int rc = cg_native<float>(c32, mu, c32->psi_n, c32->out_n, inner_tol, max_inner, &it, &rel32, 1);
+        const int rc = cg_native<float>(c32, mu, c32->psi_n, c32->out_n, inner_tol, max_inner, &it, &rel32, 1, chir);
         if (rc != OVL_OK && rc != OVL_ENOTCONV) return fail(c, rc, "inner fp32 CG: %s", c32->err);
         inner_total += it;
         k_axpy_mixed<float, double><<<gridv, BLAS_THREADS, 0, c->st>>>(n, rn, (const float2 *)c32->out_n, (double2 *)x_n);
         OVL_LAUNCH_CHECK(c);
         // r = b - A64 x
-        OVL_TRY(overlap_native<double>(c, mu, 0, x_n, c->cg_q));
-        OVL_TRY(overlap_native<double>(c, mu, 1, c->cg_q, c->cg_Ap));
+        if (chir) {
+            OVL_TRY(sign_combine_native<double>(c, 1, 0.5 * (1.0 + mu * mu), 0.5 * chir * (1.0 - mu * mu), 0, 0, x_n, c->cg_Ap, chir));
+        } else {
+            OVL_TRY(overlap_native<double>(c, mu, 0, x_n, c->cg_q));
+            OVL_TRY(overlap_native<double>(c, mu, 1, c->cg_q, c->cg_Ap));
+        }
         k_sub<double><<<gridv, BLAS_THREADS, 0, c->st>>>(n, (const double2 *)b_n, (const double2 *)c->cg_Ap, (double2 *)c->cg_r);
         OVL_LAUNCH_CHECK(c);
         OVL_TRY(reduce_redot<double>(c, c->cg_r, c->cg_r, 3, 1));

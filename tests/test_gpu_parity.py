@@ -813,6 +813,48 @@ def test_cg_chiral_sector(torch, api, orc, chir):
     assert rel_err(host(xf), host(x)) < 1e-3                                # kappa * 1/4 (1-mu)^2 * 2 delta
 
 
+@pytest.mark.parametrize("chir", [+1, -1])
+def test_cg_mixed_chiral(torch, api, orc, chir):
+    """ovl_cg_mixed_chiral: the chiral-sector system A_c x = P_c b (R23) by defect correction with fp32 inner solves.  A true
+    fp64 residual of 1e-11 -- below what fp32 can represent -- the oracle's chiral-sector CG solution, x = P_c x exactly, the
+    reported residual recomputed through the public fp64 operator (A_c from one ovl_sign), and half the stencil launches of
+    ovl_cg_mixed on the projected source."""
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 4, 8)
+    U = inputs.config_links(dims, 0.3, 177, stout_steps=1)
+    alpha = inputs.chebyshev_sign_coeffs(61, 0.09)
+    phi = inputs.orthonormal_vectors(dims, 3, 178)
+    lam = np.array([0.45, -0.47, 0.5])
+    b = inputs.gaussian_spinor(dims, 179)
+    mu = 0.2
+    g5v = G5[None, :, None]
+    xo, ito, relo = orc.cg_chiral(dims, U, alpha, mu, chir, b, 1e-11, 500, phi, lam)
+    with api.Overlap(dims, dev(torch, U), "f64") as op, api.Overlap(dims, dev(torch, U), "f32") as op32:
+        for o in (op, op32):
+            o.set_chebyshev(alpha)
+            o.set_deflation(dev(torch, phi), lam)
+        bd = dev(torch, b)
+        l0 = op.launch_count() + op32.launch_count()
+        x, no, ni, rel, ok = op.cg_mixed_chiral(op32, bd, mu, chir, tol=1e-11, inner_tol=1e-4)
+        l1 = op.launch_count() + op32.launch_count()
+        assert ok and rel <= 1e-11 and 2 <= no <= 6
+        assert rel_err(host(x), xo) < 1e-8
+        assert np.abs(0.5 * (1 - chir * g5v) * host(x)).max() == 0.0
+        pc = dev(torch, 0.5 * (1 + chir * g5v) * np.ones_like(b))
+        pb = pc * bd
+        acx = 0.5 * (1 + mu * mu) * x + 0.5 * chir * (1 - mu * mu) * pc * op.sign(x)
+        assert abs(float(torch.linalg.norm(pb - acx) / torch.linalg.norm(pb)) - rel) < 1e-13
+        xf, nof, nif, relf, okf = op.cg_mixed(op32, pb, mu, tol=1e-11, inner_tol=1e-4)
+        l2 = op.launch_count() + op32.launch_count()
+        assert okf and (l1 - l0) / max(ni, 1) < 0.6 * (l2 - l1) / max(nif, 1)
+        out = torch.empty_like(bd)
+        with pytest.raises(B.OvlError) as e:
+            B.ovl_cg_mixed_chiral(op.ctx, op32.ctx, mu, 0, bd, out, 1e-8, 1e-4, 5, 100)
+        assert e.value.code == B.OVL_EINVAL
+        with pytest.raises(B.OvlError):
+            B.ovl_cg_mixed_chiral(op32.ctx, op.ctx, mu, chir, bd, out, 1e-8, 1e-4, 5, 100)
+
+
 def test_cg_chiral_argument_checks(torch, api):
     from paper_1510_06897_b200 import binding as B
     dims = (4, 4, 4, 4)
