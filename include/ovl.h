@@ -185,6 +185,13 @@ int ovl_cg_chiral(ovl_ctx *ctx, double mu, int chirality, const void *b, void *x
 int ovl_cg_multi(ovl_ctx *ctx, int nrhs, double mu, const void *b, void *x, double tol, int maxiter, int *iters_out,
                  double *true_relres_out);
 
+/* ovl_cg_multi in one chirality sector: nrhs systems A_c x_r = P_c b_r (ovl_cg_chiral) in lockstep, one multi-right-hand-
+ * side sign application per iteration.  The spin-colour point sources of a propagator are chirality
+ * eigenstates: six of the twelve go through chirality +1, six through -1.  Arguments, outputs and errors as ovl_cg_multi;
+ * OVL_EINVAL for chirality not +-1.  Synchronises. */
+int ovl_cg_multi_chiral(ovl_ctx *ctx, int nrhs, double mu, int chirality, const void *b, void *x, double tol, int maxiter,
+                        int *iters_out, double *true_relres_out);
+
 /* Mixed-precision CG on D^dag D x = b ("10^-13 for overlap fermions (using mixed precision)"; SURVEY.md
  * §8(f) rank 2): defect correction x <- x + A32^{-1}(b - A64 x).  ctx64 is an OVL_F64 context and carries b, x (canonical
  * complex128 [H|D]), the outer fp64 residuals and the final accuracy; ctx32 is an OVL_F32 context on the same lattice and

@@ -136,6 +136,13 @@ class Overlap:
         rc, it, rel = B.ovl_cg_multi(self.ctx, int(b.shape[0]), mu, b, x, tol, maxiter)
         return x, it, rel, rc == B.OVL_OK
 
+    def cg_multi_chiral(self, b, mu, chirality, tol=1e-8, maxiter=1000):
+        """b: (nrhs, V, 4, 3). The chiral-sector systems A_c x_r = P_c b_r in lockstep (one sign application per iteration).
+        Returns (x, iterations[], true relres[], converged)."""
+        x = self._like(b)
+        rc, it, rel = B.ovl_cg_multi_chiral(self.ctx, int(b.shape[0]), mu, chirality, b, x, tol, maxiter)
+        return x, it, rel, rc == B.OVL_OK
+
     def cg_mixed(self, inner, b, mu, tol=1e-8, inner_tol=1e-4, max_outer=20, max_inner=1000):
         """Mixed-precision CG: self is the fp64 operator, `inner` an fp32 Overlap on the same lattice and stream.
         Returns (x, outer steps, fp32 iterations, true fp64 relres, converged)."""

@@ -46,6 +46,7 @@ SIGNATURES = {
     "ovl_cg": (_I, [_P, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_chiral": (_I, [_P, _D, _I, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_multi": (_I, [_P, _I, _D, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
+    "ovl_cg_multi_chiral": (_I, [_P, _I, _D, _I, _P, _P, _D, _I, C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_mixed": (_I, [_P, _P, _D, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
     "ovl_cg_mixed_chiral": (_I, [_P, _P, _D, _I, _P, _P, _D, _D, _I, _I, C.POINTER(_I), C.POINTER(_I), C.POINTER(_D)]),
     "ovl_lowest_eigenpairs": (_I, [_P, _I, _D, _I, _I, _I, _P, C.POINTER(_D), C.POINTER(_D), C.POINTER(_I)]),
@@ -248,6 +249,14 @@ def ovl_cg_multi(ctx, nrhs, mu, b, x, tol, maxiter):
     """Returns (status, iterations per system, true relative residual per system)."""
     it, rel = (_I * nrhs)(), (_D * nrhs)()
     rc = load_library().ovl_cg_multi(ctx, int(nrhs), float(mu), _ptr(b), _ptr(x), float(tol), int(maxiter), it, rel)
+    _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
+    return rc, list(it), list(rel)
+
+
+def ovl_cg_multi_chiral(ctx, nrhs, mu, chirality, b, x, tol, maxiter):
+    """Returns (status, iterations per system, true relative residual per system) of the chiral-sector systems."""
+    it, rel = (_I * nrhs)(), (_D * nrhs)()
+    rc = load_library().ovl_cg_multi_chiral(ctx, int(nrhs), float(mu), int(chirality), _ptr(b), _ptr(x), float(tol), int(maxiter), it, rel)
     _check(ctx, rc, ok=(OVL_OK, OVL_ENOTCONV))
     return rc, list(it), list(rel)
 

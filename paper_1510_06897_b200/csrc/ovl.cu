@@ -464,6 +464,26 @@ int ovl_cg_multi(ovl_ctx *c, int nrhs, double mu, const void *b, void *x, double
     return rc;
 }
 
+int ovl_cg_multi_chiral(ovl_ctx *c, int nrhs, double mu, int chirality, const void *b, void *x, double tol, int maxiter, int *iters_out,
+                        double *relres_out) {
+    if (!c) return OVL_EINVAL;
+    if (!b || !x || b == x || !iters_out || !relres_out || maxiter < 0 || (chirality != 1 && chirality != -1))
+        return fail(c, OVL_EINVAL, "bad ovl_cg_multi_chiral arguments (chirality must be +1 or -1)");
+    if (nrhs < 1 || nrhs > OVL_MAX_RHS) return fail(c, OVL_EINVAL, "nrhs must be in 1..%d", OVL_MAX_RHS);
+    if (c->alpha.empty()) return fail(c, OVL_ESTATE, "ovl_set_chebyshev has not been called");
+    OVL_TRY(ensure_multi_staging(c, nrhs));
+    const size_t cb = c->canon_bytes(), fb = c->field_bytes();
+    for (int r = 0; r < nrhs; ++r) OVL_TRY(import_any(c, (const char *)b + r * cb, (char *)c->multi_in + r * fb));
+    int rc = DISPATCH(c, cg_native, c, mu, c->multi_in, c->multi_out, tol, maxiter, iters_out, relres_out, nrhs, chirality);
+    if (rc != OVL_OK && rc != OVL_ENOTCONV) return rc;
+    for (int r = 0; r < nrhs; ++r) {
+        int rc2 = export_any(c, (const char *)c->multi_out + r * fb, (char *)x + r * cb);
+        if (rc2 != OVL_OK) return rc2;
+    }
+    OVL_CUDA(c, cudaStreamSynchronize(c->st));
+    return rc;
+}
+
 int ovl_cg_mixed(ovl_ctx *c, ovl_ctx *c32, double mu, const void *b, void *x, double tol, double inner_tol, int max_outer,
                  int max_inner, int *outer_out, int *inner_out, double *relres_out) {
     if (!c || !c32) return OVL_EINVAL;

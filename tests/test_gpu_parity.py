@@ -855,6 +855,33 @@ def test_cg_mixed_chiral(torch, api, orc, chir):
             B.ovl_cg_mixed_chiral(op32.ctx, op.ctx, mu, chir, bd, out, 1e-8, 1e-4, 5, 100)
 
 
+def test_cg_multi_chiral(torch, api, orc):
+    """ovl_cg_multi_chiral: several chiral-sector systems in lockstep -- every solution bit-identical to the single-system
+    ovl_cg_chiral, one of them against the oracle's chiral-sector CG, a source with P_c b = 0 among the others returns
+    x = 0 after 0 iterations."""
+    dims = (4, 4, 6, 8)
+    U = inputs.config_links(dims, 0.3, 21, stout_steps=2)
+    alpha = inputs.chebyshev_sign_coeffs(101, 0.07)
+    phi = inputs.orthonormal_vectors(dims, 3, 23)
+    lam = np.array([0.5, -0.51, 0.52])
+    mu, chir = 0.1, -1
+    bs = np.stack([inputs.gaussian_spinor(dims, 300 + r) for r in range(4)])
+    bs[2] = 0.5 * (1 - chir * G5[None, :, None]) * bs[2]        # lives entirely in the other sector: P_c b = 0
+    with api.Overlap(dims, dev(torch, U)) as op:
+        op.set_chebyshev(alpha)
+        op.set_deflation(dev(torch, phi), lam)
+        bd = dev(torch, bs)
+        x, it, rel, ok = op.cg_multi_chiral(bd, mu, chir, tol=1e-9, maxiter=500)
+        singles = [op.cg_chiral(bd[r].contiguous(), mu, chir, tol=1e-9, maxiter=500) for r in range(4)]
+    assert ok and it[2] == 0 and float(torch.abs(x[2]).max()) == 0.0
+    for r in range(4):
+        assert torch.equal(x[r], singles[r][0]) and it[r] == singles[r][1]
+        if r != 2:
+            assert rel[r] < 1.05e-9
+    xo, ito, relo = orc.cg_chiral(dims, U, alpha, mu, chir, bs[1], 1e-9, 500, phi, lam)
+    assert abs(it[1] - ito) <= 2 and rel_err(host(x[1]), xo) < 1e-6
+
+
 def test_cg_chiral_argument_checks(torch, api):
     from paper_1510_06897_b200 import binding as B
     dims = (4, 4, 4, 4)
