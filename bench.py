@@ -512,9 +512,21 @@ def bench_cg_mixed(torch, api, w, host_inputs=None, tol=1e-8, inner_tol=1e-4, la
         xc, noc, nic, relc, okc = op.cg_mixed_chiral(op32, bd, 0.05, +1, tol=tol, inner_tol=inner_tol)
         torch.cuda.synchronize()
         dtc = time.perf_counter() - t0
+        # ... and with a relaxed inner sign function ("relaxed"): half the polynomial degree in the fp32 context only;
+        # the fp64 outer residuals keep the full-degree operator, so the answer meets the same tol for the same system
+        relaxed = {}
+        if w["degree"] >= 100:
+            op32.set_chebyshev(inputs.chebyshev_sign_coeffs(w["degree"] // 2, w["poly_eps"]))
+            t0 = time.perf_counter()
+            xr, nor, nir, relr, okr = op.cg_mixed_chiral(op32, bd, 0.05, +1, tol=tol, inner_tol=inner_tol)
+            torch.cuda.synchronize()
+            relaxed = {"inner_degree": w["degree"] // 2, "seconds": time.perf_counter() - t0, "outer_steps": nor, "fp32_iterations": nir,
+                       "true_relres": relr, "converged": okr,
+                       "rel_diff_to_full_degree_inner": float(torch.linalg.norm(xr - xc) / torch.linalg.norm(xc))}
     return {"workload": label, "mixed_seconds": dt, "outer_steps": no, "fp32_iterations": ni, "true_relres": rel, "converged": ok,
             "fp64_seconds": dt64, "fp64_iterations": it64, "fp64_true_relres": rel64, "rel_diff_of_solutions": diff,
-            "mixed_chiral_sector": {"seconds": dtc, "outer_steps": noc, "fp32_iterations": nic, "true_relres": relc, "converged": okc}}
+            "mixed_chiral_sector": {"seconds": dtc, "outer_steps": noc, "fp32_iterations": nic, "true_relres": relc, "converged": okc,
+                                    "relaxed_inner_sign": relaxed}}
 
 
 def bench_true_eigenpairs(torch, api, w, host_inputs, steps, warmup, block=104, degree=200):
