@@ -742,10 +742,10 @@ def run_native(args, w):
         if args.workload == "cfg3":
             w1 = dict(WORKLOADS["cfg1"], name="cfg1")
             r1 = bench_overlap(torch, api, B, w1, "f64", 18, 20, 5, None, 0, False)
-            r1p = bench_overlap(torch, api, B, w1, "f64", 18, 20, 5, None, 0, False, variant="plain")
+            r1b = bench_overlap(torch, api, B, w1, "f64", 18, 20, 5, None, 0, False, variant="brick")
             extras["cfg1_8x8x8x32"] = {"applies_per_s": r1["applies_per_s"], "us_per_order": r1["kernel_us"],
-                                        "orders": r1["orders"], "site_order": "brick (default for V <= 2^18)",
-                                        "plain_site_order": {"applies_per_s": r1p["applies_per_s"], "us_per_order": r1p["kernel_us"]}}
+                                        "orders": r1["orders"], "site_order": "plain (the default outside 2^15 <= V <= 2^17)",
+                                        "brick_site_order": {"applies_per_s": r1b["applies_per_s"], "us_per_order": r1b["kernel_us"]}}
             extras["cfg2_cg"] = bench_cg(torch, api, w1)
             extras["cfg1_eigensolver"] = bench_eigensolver(torch, api, w1, 20, 40, 200)
             if args.cfg3_eigensolver:  # ~40 s: the 50 pairs of config 3 (block 104 reaches past the 24 + 72 clusters)

@@ -75,9 +75,9 @@ class Overlap:
         B.ovl_set_recurrence(self.ctx, m)
 
     def set_fused_variant(self, variant):
-        """'register' (default; brick order on small lattices), 'plain' (register kernel, plain site order) or 'bulk' (cp.async.bulk
+        """'register' (default; picks the site order by lattice size), 'plain' / 'brick' (register kernel, that site order) or 'bulk' (cp.async.bulk
         landing zone for the links): same results bit for bit, see include/ovl.h."""
-        v = {"register": B.OVL_FUSED_REGISTER, "bulk": B.OVL_FUSED_BULK, "plain": B.OVL_FUSED_PLAIN}.get(variant, variant)
+        v = {"register": B.OVL_FUSED_REGISTER, "bulk": B.OVL_FUSED_BULK, "plain": B.OVL_FUSED_PLAIN, "brick": B.OVL_FUSED_BRICK}.get(variant, variant)
         B.ovl_set_fused_variant(self.ctx, v)
 
     def set_graphs(self, on=True):

@@ -15,7 +15,7 @@ OVL_OK, OVL_EINVAL, OVL_ENOMEM, OVL_ECUDA, OVL_ESTATE, OVL_ENOTCONV = range(6)
 OVL_F64, OVL_F32 = 0, 1
 OVL_RECON18, OVL_RECON12 = 18, 12
 OVL_REC_CLENSHAW, OVL_REC_FORWARD = 0, 1
-OVL_FUSED_REGISTER, OVL_FUSED_BULK, OVL_FUSED_PLAIN = 0, 1, 2
+OVL_FUSED_REGISTER, OVL_FUSED_BULK, OVL_FUSED_PLAIN, OVL_FUSED_BRICK = 0, 1, 2, 3
 OVL_MAX_RHS = 12
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

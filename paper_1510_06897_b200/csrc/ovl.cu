@@ -150,12 +150,14 @@ int create_impl(ovl_ctx **out, const int dims[4], const void *links_c128, int pr
             if (best > 0 && best < dims[2]) { c->sweep.tpc = c->g.sxy * best / 128; c->sweep.nzs = dims[2] / best; }
         }
     }
-    // brick order (ovl_types.cuh): lattices up to 2^18 sites (8^4 ... 16^3 x 32: a launch is bound by the per-SM L2 -> L1 fill
-    // rate; measured -8 ... -15 % per order, neutral from 20^3 x 64 on), Lz and Lt even
-    if (c->g.V <= (1 << 18) && dims[2] % 2 == 0 && dims[3] % 2 == 0) {
-        c->brick.half = c->g.sxyz / 2;
-        c->brick.nchunk = (c->brick.half + ovl::BRICK_GS - 1) / ovl::BRICK_GS;
+    // brick order (ovl_types.cuh): possible whenever Lz and Lt are even (brick_geom); chosen by default for 2^15 <= V <= 2^17
+    // (12^3 x 24 ... 16^3 x 32: -2 ... -5 % per order; smaller lattices are faster in plain order, 8^3 x 32 4.6 against 5.0 us,
+    // from 16^3 x 48 on there is no difference)
+    if (dims[2] % 2 == 0 && dims[3] % 2 == 0) {
+        c->brick_geom.half = c->g.sxyz / 2;
+        c->brick_geom.nchunk = (c->brick_geom.half + ovl::BRICK_GS - 1) / ovl::BRICK_GS;
     }
+    if (c->g.V >= (1 << 15) && c->g.V <= (1 << 17)) c->brick = c->brick_geom;
     c->brick_auto = c->brick;
     c->prec = prec;
     c->recon = recon;
@@ -339,10 +341,11 @@ int ovl_get_recurrence(const ovl_ctx *c) { return c ? c->recurrence : -1; }
 
 int ovl_set_fused_variant(ovl_ctx *c, int variant) {
     if (!c) return OVL_EINVAL;
-    if (variant != OVL_FUSED_REGISTER && variant != OVL_FUSED_BULK && variant != OVL_FUSED_PLAIN)
+    if (variant != OVL_FUSED_REGISTER && variant != OVL_FUSED_BULK && variant != OVL_FUSED_PLAIN && variant != OVL_FUSED_BRICK)
         return fail(c, OVL_EINVAL, "unknown fused-kernel variant %d", variant);
+    if (variant == OVL_FUSED_BRICK && c->brick_geom.nchunk == 0) return fail(c, OVL_EINVAL, "brick order needs Lz and Lt even");
     c->fused_variant = variant;
-    c->brick = variant == OVL_FUSED_PLAIN ? ovl::Brick{0, 0} : c->brick_auto;
+    c->brick = variant == OVL_FUSED_PLAIN ? ovl::Brick{0, 0} : variant == OVL_FUSED_BRICK ? c->brick_geom : c->brick_auto;
     ++c->poly_gen;  // captured graphs hold the other kernel
     return OVL_OK;
 }

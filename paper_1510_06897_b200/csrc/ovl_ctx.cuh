@@ -16,6 +16,7 @@ struct ovl_ctx {
     ovl::Sweep sweep{0, 0};  // L2-aware tile order (tpc = 0: plain order)
     ovl::Brick brick{0, 0};  // brick order for small lattices (nchunk = 0: plain order)
     ovl::Brick brick_auto{0, 0};  // what create chose (OVL_FUSED_PLAIN switches `brick` off, OVL_FUSED_REGISTER restores it)
+    ovl::Brick brick_geom{0, 0};  // the brick decomposition of this lattice if it has one (OVL_FUSED_BRICK forces it)
     int prec = OVL_F64, recon = OVL_RECON18, recurrence = OVL_REC_CLENSHAW, fused_variant = OVL_FUSED_REGISTER;
     int sm_count = 148;
     cudaStream_t st = nullptr;

@@ -15,11 +15,14 @@ namespace ovl {
         if (e_ != cudaSuccess) return fail((c), OVL_ECUDA, "kernel launch: %s", cudaGetErrorString(e_)); \
     } while (0)
 
-// launch shape of the fused kernel: 128-thread CTAs (tiles of 128 consecutive sites); fp64 runs 3 CTAs/SM at up to 168
-// registers, fp32 4 CTAs/SM (measured best on B200)
+// launch shape of the fused kernel: 128-thread CTAs (tiles of 128 consecutive sites).  Several right-hand sides, the L2-aware
+// sweep and the t-split slabs: fp64 3 CTAs/SM at up to 168 registers, fp32 4 CTAs/SM.  The single-right-hand-side fp64 kernel
+// (MINB_SINGLE): 2 CTAs/SM, up to 255 registers, no spills -- at boost clocks the same speed as 3 CTAs/SM (ptxas turns the
+// registers into deeper load batches), under the power cap of a long run and together with the evict-first loads of the
+// single-use streams 3 % faster (A/B on one box: 130.1 -> 126.0 us/order)
 template <typename T> struct WilsonCfg;
-template <> struct WilsonCfg<double> { static constexpr int THREADS = 128, MINB = 3; };
-template <> struct WilsonCfg<float> { static constexpr int THREADS = 128, MINB = 4; };
+template <> struct WilsonCfg<double> { static constexpr int THREADS = 128, MINB = 3, MINB_SINGLE = 2; };
+template <> struct WilsonCfg<float> { static constexpr int THREADS = 128, MINB = 4, MINB_SINGLE = 4; };
 
 struct WilsonArgs {
     const void *in = nullptr, *prev = nullptr, *psi = nullptr;
@@ -73,7 +76,7 @@ template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx 
         k_wilson_fused_swept<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
             c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp, c->sweep);
     else
-        k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
+        k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB_SINGLE><<<grid, TH, 0, c->st>>>(
             c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp);
 }
 

@@ -78,6 +78,35 @@ __device__ __forceinline__ int brick_site(const Brick &bk, const Geom &g, int ct
 __device__ __forceinline__ double2 ldg(const double2 *p) { return __ldg(p); }
 __device__ __forceinline__ float2 ldg(const float2 *p) { return __ldg(p); }
 
+// loads of single-use streams (b_{k+2}, psi: read once per launch, no neighbour reuse): L2 evict-first, so that they do not
+// displace the stencil operand and the links, which the neighbouring sites and the backward hops find in L2
+__device__ __forceinline__ unsigned long long l2_evict_first_policy() {
+    unsigned long long p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ double2 ldg_once(const double2 *p) {
+    double2 v;
+    asm("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(l2_evict_first_policy()));
+    return v;
+}
+__device__ __forceinline__ float2 ldg_once(const float2 *p) {
+    float2 v;
+    asm("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(l2_evict_first_policy()));
+    return v;
+}
+// the same for a field the kernel also writes (coherent load, ordered against the store of the same thread)
+__device__ __forceinline__ double2 ld_once(const double2 *p) {
+    double2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(l2_evict_first_policy()) : "memory");
+    return v;
+}
+__device__ __forceinline__ float2 ld_once(const float2 *p) {
+    float2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(l2_evict_first_policy()) : "memory");
+    return v;
+}
+
 // 16- or 8-byte asynchronous global -> shared copy of one complex (LDGSTS), and its completion wait
 template <typename C> __device__ __forceinline__ void cp_async_cx(C *smem, const C *gmem) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);

@@ -211,7 +211,7 @@ __device__ __forceinline__ void wilson_site(const Geom &g, const cx<T> *__restri
     if (FLAGS & K_PREV) {
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const cx<T> pv = prev[k * V + s];  // ld.global (not .nc): out may alias prev
+            const cx<T> pv = ld_once(prev + k * V + s);  // coherent load (not .nc): out may alias prev
             const T r = ((FLAGS & K_G5) && k >= 6) ? sp.r_p : -sp.r_p;
             hop[k].x = fma(r, pv.x, hop[k].x);
             hop[k].y = fma(r, pv.y, hop[k].y);
@@ -220,7 +220,7 @@ __device__ __forceinline__ void wilson_site(const Geom &g, const cx<T> *__restri
     if (FLAGS & K_PSI) {
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const cx<T> ps = ldg(psi + k * V + s);
+            const cx<T> ps = ldg_once(psi + k * V + s);
             const T r = ((FLAGS & K_G5) && k >= 6) ? -sp.r_a : sp.r_a;
             hop[k].x = fma(r, ps.x, hop[k].x);
             hop[k].y = fma(r, ps.y, hop[k].y);

@@ -930,14 +930,13 @@ def test_bulk_copy_variant_bit_identical(torch, api, orc, prec, recon, dims):
 
 
 @pytest.mark.parametrize("prec,recon", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
-@pytest.mark.parametrize("dims", [(8, 8, 8, 32), (4, 6, 8, 10), (6, 4, 2, 8), (2, 2, 2, 2), (10, 6, 4, 12), (8, 8, 8, 8)])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 32), (4, 6, 8, 10), (6, 4, 2, 8), (2, 2, 2, 2), (10, 6, 4, 12), (8, 8, 8, 8), (12, 12, 12, 24)])
 def test_brick_order_bit_identical_to_plain_order(torch, api, orc, prec, recon, dims):
-    """Lattices of at most 2^18 sites with Lz, Lt even run their single-right-hand-side launches in brick order by default
-    (k_wilson_fused_brick: a CTA takes a 2 x 2 stack in (z, t) of 32-site chunks).  OVL_FUSED_PLAIN forces the plain tile
-    order of the large-lattice kernel on the same lattice: D_W, K^, the deflated sign function in both recurrences and
-    D^dag must agree bit for bit -- ragged chunks (V/2 not a multiple of 32 per time-slice pair), extent-2 directions,
-    non-cubic shapes -- and the plain-order result is held against the oracle (the large-lattice kernel's edge handling
-    is otherwise only reached at 20^3 x 64 and above)."""
+    """Brick order (k_wilson_fused_brick: a CTA takes a 2 x 2 stack in (z, t) of 32-site chunks; the default for
+    2^15 <= V <= 2^17, forced here with OVL_FUSED_BRICK) against the plain tile order (OVL_FUSED_PLAIN) on the same lattice:
+    D_W, K^, the deflated sign function in both recurrences and D^dag must agree bit for bit -- ragged chunks (V/2 not a
+    multiple of 32 per time-slice pair), extent-2 directions, non-cubic shapes -- and the plain-order result is held
+    against the oracle."""
     U = inputs.config_links(dims, 0.4, 61, stout_steps=1)
     psi = inputs.gaussian_spinor(dims, 62)
     alpha = rough_alpha(17, seed=9)
@@ -956,6 +955,8 @@ def test_brick_order_bit_identical_to_plain_order(torch, api, orc, prec, recon, 
         op.set_chebyshev(alpha)
         op.set_deflation(dev(torch, phi), lam)
         p = dev(torch, psi, op.cdtype)
+        default = op.sign(p)
+        op.set_fused_variant("brick")
         brick = run(op, p)
         op.set_fused_variant("plain")
         plain = run(op, p)
@@ -963,7 +964,7 @@ def test_brick_order_bit_identical_to_plain_order(torch, api, orc, prec, recon, 
         back = op.sign(p)
     for b_, p_ in zip(brick, plain):
         assert torch.equal(b_, p_)
-    assert torch.equal(back, brick[2])
+    assert torch.equal(back, brick[2]) and torch.equal(default, brick[2])
     tol = TOL_OVL if prec == "f64" else TOL_F32
     assert rel_err(host(plain[0]).astype(np.complex128), orc.dw(dims, U, psi)) < (TOL_DW if prec == "f64" else TOL_F32)
     assert rel_err(host(plain[2]).astype(np.complex128), orc.sign(dims, U, alpha, psi, phi, lam)) < tol
