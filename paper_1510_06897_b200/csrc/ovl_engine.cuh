@@ -75,8 +75,11 @@ template <typename T, int RECON, int FLAGS> inline void launch_wilson_t(ovl_ctx 
     else if (c->sweep.tpc > 0)
         k_wilson_fused_swept<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
             c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp, c->sweep);
-    else
+    else if ((FLAGS & K_PREV) || c->g.V <= (1 << 18))
         k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB_SINGLE><<<grid, TH, 0, c->st>>>(
+            c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp);
+    else  // no b_{k+2} stream (D_W, K^, the first two Clenshaw launches) on a large lattice: 3 CTAs/SM is 3 % faster at boost clocks
+        k_wilson_fused<T, RECON, FLAGS, TH, WilsonCfg<T>::MINB><<<grid, TH, 0, c->st>>>(
             c->g, (const cx<T> *)c->U, (const cx<T> *)a.in, (const cx<T> *)a.prev, (const cx<T> *)a.psi, (cx<T> *)a.out, (cx<T> *)a.acc, sp);
 }
 
