@@ -733,6 +733,10 @@ def test_caller_owned_workspace(torch, api, orc):
         x = torch.empty_like(pd)
         xs = torch.empty_like(pd[0])
         ev = torch.empty((4, int(np.prod(dims)), 4, 3), dtype=torch.complex128, device="cuda")
+        # every kernel once on the library-owned context first: the driver loads a kernel's code on its first launch (CUDA
+        # lazy loading) and takes device memory for it, which is not an allocation of the library
+        ref.overlap_multi(pd, 0.05); ref.cg(pd[0], 0.2, tol=1e-9, maxiter=3); ref.cg_multi(pd, 0.2, tol=1e-9, maxiter=3)
+        ref.overlap(psi[1], 0.05); ref.lowest_eigenpairs(4, tol=1e-8, max_cycles=60, filter_degree=40, block=12)
         alloc1 = torch.cuda.memory_allocated()
         torch.cuda.synchronize()
         free1, _ = torch.cuda.mem_get_info()
@@ -880,6 +884,43 @@ def test_cg_multi_chiral(torch, api, orc):
             assert rel[r] < 1.05e-9
     xo, ito, relo = orc.cg_chiral(dims, U, alpha, mu, chir, bs[1], 1e-9, 500, phi, lam)
     assert abs(it[1] - ito) <= 2 and rel_err(host(x[1]), xo) < 1e-6
+
+
+def test_workspace_contexts_mixed_precision_calls(torch, api):
+    """The calls that pair an fp64 with an fp32 context (ovl_cg_mixed_chiral, ovl_lowest_eigenpairs_mixed) and the chiral
+    lockstep solver, with BOTH contexts inside torch-owned workspaces: no device allocation behind torch's back, results
+    bit-identical to library-owned contexts."""
+    from paper_1510_06897_b200 import binding as B
+    dims = (4, 4, 6, 8)
+    U = inputs.config_links(dims, 0.3, 41, stout_steps=1)
+    alpha = inputs.chebyshev_sign_coeffs(41, 0.09)
+    phi = inputs.orthonormal_vectors(dims, 4, 43)
+    lam = np.array([0.45, -0.47, 0.5, -0.52])
+    psi = np.stack([inputs.gaussian_spinor(dims, 50 + r) for r in range(3)])
+    Ud, phid, pd = dev(torch, U), dev(torch, phi), dev(torch, psi)
+    caps = dict(max_nev=4, max_rhs=3, eig_block=12)
+    with api.Overlap(dims, Ud) as r64, api.Overlap(dims, Ud, "f32") as r32, \
+            api.Overlap(dims, Ud, workspace=dict(caps)) as w64, api.Overlap(dims, Ud, "f32", workspace=dict(caps)) as w32:
+        for o in (r64, r32, w64, w32):
+            o.set_chebyshev(alpha)
+            o.set_deflation(phid, lam)
+        x1, x2 = torch.empty_like(pd[0]), torch.empty_like(pd)
+        ev = torch.empty((4, int(np.prod(dims)), 4, 3), dtype=torch.complex128, device="cuda")
+        # reference results first: they also load every kernel's code (CUDA lazy loading takes device memory per kernel)
+        y1, _, _, _, ok1 = r64.cg_mixed_chiral(r32, pd[0], 0.2, +1, tol=1e-10, inner_tol=1e-4, max_outer=10, max_inner=200)
+        y2, _, _, ok2 = r64.cg_multi_chiral(pd, 0.2, -1, tol=1e-9, maxiter=200)
+        pr, lr, _, _, _, ok3 = r64.lowest_eigenpairs_mixed(r32, 4, tol=1e-8, max_cycles=60, filter_degree=40, block=12)
+        torch.cuda.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        rc1, no, ni, rel = B.ovl_cg_mixed_chiral(w64.ctx, w32.ctx, 0.2, +1, pd[0], x1, 1e-10, 1e-4, 10, 200)
+        rc2, its, rels = B.ovl_cg_multi_chiral(w64.ctx, 3, 0.2, -1, pd, x2, 1e-9, 200)
+        rc3, lam_e, res_e, cyc, c32 = B.ovl_lowest_eigenpairs_mixed(w64.ctx, w32.ctx, 4, 1e-8, 60, 40, 12, ev)
+        torch.cuda.synchronize()
+        free2, _ = torch.cuda.mem_get_info()
+        assert free2 == free1, "the library allocated device memory behind torch's back"
+        assert rc1 == rc2 == rc3 == B.OVL_OK and rel <= 1e-10 and c32 >= 1
+        assert ok1 and ok2 and ok3
+        assert torch.equal(x1, y1) and torch.equal(x2, y2) and np.array_equal(lam_e, lr) and torch.equal(ev, pr)
 
 
 def test_cg_chiral_argument_checks(torch, api):
