@@ -886,6 +886,22 @@ def test_cg_multi_chiral(torch, api, orc):
     assert abs(it[1] - ito) <= 2 and rel_err(host(x[1]), xo) < 1e-6
 
 
+def test_fused_variant_argument_checks(torch, api):
+    from paper_1510_06897_b200 import binding as B
+    dims = (5, 3, 7, 3)     # Lz, Lt odd: no brick decomposition
+    with api.Overlap(dims, inputs.random_links(dims, 0.3, 5)) as op:
+        with pytest.raises(B.OvlError) as e:
+            op.set_fused_variant("brick")
+        assert e.value.code == B.OVL_EINVAL
+        with pytest.raises(B.OvlError) as e:
+            op.set_fused_variant(7)
+        assert e.value.code == B.OVL_EINVAL
+        for v in ("plain", "bulk", "register"):
+            op.set_fused_variant(v)
+        p = dev(torch, inputs.gaussian_spinor(dims, 6))
+        assert torch.isfinite(torch.view_as_real(op.dw(p))).all()
+
+
 def test_workspace_contexts_mixed_precision_calls(torch, api):
     """The calls that pair an fp64 with an fp32 context (ovl_cg_mixed_chiral, ovl_lowest_eigenpairs_mixed) and the chiral
     lockstep solver, with BOTH contexts inside torch-owned workspaces: no device allocation behind torch's back, results
