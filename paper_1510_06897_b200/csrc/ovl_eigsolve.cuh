@@ -279,7 +279,8 @@ inline int eig_lowest(ovl_ctx *c, ovl_ctx *c32, int nev, double tol, int max_cyc
     if ((size_t)m > n) return fail(c, OVL_EINVAL, "block size %d exceeds the dimension of the space", m);
     if (degree < 1) degree = 1;
     const int cap = std::max(m, 2 * nev);  // vectors per work block
-    const int chunk = std::min(m, c->ws_mode ? c->max_rhs : (int)OVL_MAX_RHS);  // vectors per filter pass (recurrence workspace)
+    int chunk = std::min(m, c->ws_mode ? c->max_rhs : (int)OVL_MAX_RHS);  // vectors per filter pass (recurrence workspace)
+    if (c32 && c32->ws_mode) chunk = std::min(chunk, c32->max_rhs);          // ... of both contexts
     OVL_TRY(ensure_work(c, chunk));
     if (c32) {
         const int rc = ensure_work(c32, chunk);
